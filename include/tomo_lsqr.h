@@ -1,0 +1,127 @@
+/* tomo_lsqr.h — C ABI of the B200-native damped sparse LSQR library (libtomolsqr.so).
+ *
+ * The operation (Eq. 6; solver family P:142, ref. P:268): solve the sparse,
+ * over-determined, regularised least-squares problem of direct surface-wave tomography
+ *
+ *        min_x  || A x - b ||^2  +  damp^2 || x ||^2 ,          A  m x n  in CSR on the device,
+ *
+ * by LSQR (Golub-Kahan bidiagonalisation, Paige & Saunders 1982) with x_0 = 0.  A stacks the
+ * traveltime-sensitivity rows (Eq. 1, Eq. 5, unknowns depth-fastest Eq. 7) on top
+ * of smoothing rows; the library itself accepts any canonical CSR matrix.  The step-by-step algorithm,
+ * the stopping rules and every reading taken where the paper is silent are in DESIGN.md.
+ *
+ * Everything runs in hand-written CUDA kernels for sm_100a (no cuSPARSE/cuBLAS, no CPU fallback):
+ * a device-side stable CSR->CSC transpose at create, fused SpMV+axpy+norm kernels for A v and A^T u,
+ * device-resident LSQR scalars, CUDA-graph replay of `check_every` iterations per host poll.
+ *
+ * Conventions
+ *   d_*  : DEVICE pointer on the current CUDA device (cudaMalloc / torch allocation).  A host pointer is
+ *          rejected with TOMO_ERR_NOT_DEVICE_PTR.  h_* and `res`, `out`: HOST pointers.
+ *   CSR  : rowptr int64[m+1] (rowptr[0]=0, rowptr[m]=nnz, non-decreasing), colind int32[nnz] with
+ *          0 <= col < n STRICTLY INCREASING inside each row (sorted, no duplicates), vals fp64[nnz] or
+ *          fp32[nnz], all finite.  1 <= m, n < 2^31, 0 <= nnz < 2^62.  colind and vals must be 16-byte
+ *          aligned.  Violations -> TOMO_ERR_BAD_CSR / TOMO_ERR_INVALID_ARG.
+ *   Ownership: the three CSR arrays are BORROWED: the caller keeps them alive and unmodified until
+ *          tomo_lsqr_destroy.  The handle owns the CSC copy, the work vectors, the scalars, the graphs.
+ *          Output arrays (d_x, d_out, d_X) are caller-allocated and fully overwritten.
+ *   Errors: status codes only; no exceptions, no abort.  On error, *out is NULL / outputs are unspecified.
+ *   Streams: `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
+ *          enqueued on it; solve* return after their last host poll, i.e. results are valid on return.
+ *   Threads: one handle runs one call at a time; different handles are independent.
+ *   Device: compute capability 10.x only (TOMO_ERR_UNSUPPORTED_ARCH otherwise; no fallback).
+ */
+#ifndef TOMO_LSQR_H_
+#define TOMO_LSQR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tomo_lsqr_s* tomo_lsqr_t; /* opaque handle */
+
+typedef enum {
+  TOMO_OK = 0,
+  TOMO_ERR_INVALID_ARG = 1,
+  TOMO_ERR_BAD_CSR = 2,
+  TOMO_ERR_NOT_DEVICE_PTR = 3,
+  TOMO_ERR_OOM = 4,
+  TOMO_ERR_CUDA = 5,
+  TOMO_ERR_UNSUPPORTED_ARCH = 6,
+  TOMO_ERR_RANGE = 7
+} tomo_status_t;
+
+typedef enum { TOMO_VAL_F64 = 0, TOMO_VAL_F32 = 1 } tomo_valtype_t;
+
+/* Filled by the solve calls (host memory).  istop: 0 = x=0 is the exact solution (b=0 or A^T b=0);
+ * 1 = ||r|| <= btol*||b|| + atol*||A||*||x||;  2 = ||A^T r|| / (||A|| ||r||) <= atol;  3 unused (no
+ * condition limit);  4,5,6 = the same three tests at machine precision;  7 = max_iters reached. */
+typedef struct {
+  int32_t itn;    /* iterations performed */
+  int32_t istop;  /* reason for stopping, see above */
+  double r1norm;  /* ||b - A x||  (from r2norm and xnorm, reading F3) */
+  double r2norm;  /* sqrt(||b - A x||^2 + damp^2 ||x||^2): the quantity LSQR decreases monotonically */
+  double arnorm;  /* ||A^T r - damp^2 x||  estimate */
+  double anorm;   /* Frobenius-type estimate of ||[A; damp I]|| */
+  double acond;   /* estimate of cond([A; damp I]) */
+  double xnorm;   /* ||x|| estimate */
+} tomo_lsqr_result_t;
+
+/* a0: validate the CSR arrays on the device, build the stable CSC transpose
+ * (rows ascending inside each column) and the nnz-balanced row / column partitions.  One-off per matrix.
+ * vt selects the storage type of d_vals (arithmetic is fp64 either way). */
+tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr,
+                               const int32_t* d_colind, const void* d_vals, tomo_valtype_t vt, void* cuda_stream);
+
+/* a1-a7: LSQR on (A, b, damp) from x_0 = 0 until a stopping test fires or max_iters iterations.
+ * d_b fp64[m], d_x fp64[n].  damp, atol, btol >= 0 and finite; max_iters >= 0 (0: x = 0, istop = 7).
+ * h_r2norm_hist / h_arnorm_hist: NULL or host fp64[max_iters]; entry k-1 = r2norm / arnorm after
+ * iteration k, for k = 1..res->itn. */
+tomo_status_t tomo_lsqr_solve(tomo_lsqr_t h, const double* d_b, double damp, double atol, double btol,
+                              int32_t max_iters, double* d_x, tomo_lsqr_result_t* res, double* h_r2norm_hist,
+                              double* h_arnorm_hist, void* cuda_stream);
+
+/* The same solve with HOST buffers: h_b fp64[m] is copied to the device, h_x fp64[n] is copied back
+ * (the end-to-end entry bench.py times; the matrix stays resident in the handle). */
+tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
+                                   int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream);
+
+/* a8: nrhs (1..8) independent LSQR recurrences sharing each pass over A / A^T (BASELINE configs[3]).
+ * d_B fp64[m x nrhs] row-major, d_X fp64[n x nrhs] row-major, res[nrhs].  Every right-hand side stops
+ * on its own tests; iterates of a stopped side are frozen. */
+tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
+                                    double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
+                                    void* cuda_stream);
+
+/* y = A x (transpose = 0: d_in fp64[n], d_out fp64[m]) or y = A^T x (transpose = 1: d_in fp64[m],
+ * d_out fp64[n]) with the kernels the solver uses (the A^T product gathers over the CSC copy). */
+tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const double* d_in, double* d_out, void* cuda_stream);
+
+/* Copy the CSC arrays built at create to caller device buffers (colptr int64[n+1], rowind int32[nnz],
+ * cvals of the handle's value type [nnz]); any pointer may be NULL to skip it.  Test/inspection hook. */
+tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_rowind, void* d_cvals, void* cuda_stream);
+
+/* Options (set between solves):
+ *   "check_every" k >= 1   iterations per graph replay / host poll (default 10); never changes results
+ *   "accumulate"  0 | 1    0 = fast: fp64 FMA sums; 1 = dd: double-double sums rounded once (default 1,
+ *                          the order-independent iterate that parity at fixed k is claimed for)
+ *   "graph"       0 | 1    replay a CUDA graph (default 1) or launch kernel by kernel
+ *   "profile"     0 | 1    1: kernel-by-kernel launches bracketed by CUDA events (see tomo_lsqr_get_info)
+ *   "waves"       w >= 1   static partitions per resident block slot (default 1) */
+tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value);
+
+/* Read-outs (host double): "create_ms", "transpose_ms", "csc_bytes", "scratch_bytes", "blocks_rows",
+ * "blocks_cols", and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
+ * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each). */
+tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, double* out);
+
+void tomo_lsqr_destroy(tomo_lsqr_t h);
+
+/* Static string for a status; for TOMO_ERR_CUDA the text of the last CUDA error seen by this thread. */
+const char* tomo_status_string(tomo_status_t s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TOMO_LSQR_H_ */

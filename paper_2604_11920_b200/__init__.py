@@ -1,0 +1,238 @@
+"""paper_2604_11920_b200 — thin Python binding of libtomolsqr.so (include/tomo_lsqr.h).
+
+Argument marshalling only: every step of the hot path (CSR->CSC transpose, A v, A^T u, norms, scalar
+recurrences, x/w update, stopping tests) runs in the library's CUDA kernels.  PyTorch supplies device
+memory and streams.  There is NO fallback: if the shared library is missing or was not built, importing
+the entry points raises.  Functions carry the names of the C ABI; :class:`TomoLsqr` is a convenience
+wrapper that keeps the borrowed CSR tensors alive.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtomolsqr.so")
+
+TOMO_OK = 0
+TOMO_ERR_INVALID_ARG, TOMO_ERR_BAD_CSR, TOMO_ERR_NOT_DEVICE_PTR, TOMO_ERR_OOM = 1, 2, 3, 4
+TOMO_ERR_CUDA, TOMO_ERR_UNSUPPORTED_ARCH, TOMO_ERR_RANGE = 5, 6, 7
+TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
+
+# every symbol include/tomo_lsqr.h declares
+SYMBOLS = (
+    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsqr_solve_host", "tomo_lsqr_solve_multi", "tomo_lsqr_spmv",
+    "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
+)
+
+
+class tomo_lsqr_result_t(ctypes.Structure):
+    _fields_ = [("itn", ctypes.c_int32), ("istop", ctypes.c_int32), ("r1norm", ctypes.c_double),
+                ("r2norm", ctypes.c_double), ("arnorm", ctypes.c_double), ("anorm", ctypes.c_double),
+                ("acond", ctypes.c_double), ("xnorm", ctypes.c_double)]
+
+
+class TomoError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: status {status} ({tomo_status_string(status)})")
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """dlopen libtomolsqr.so (built in-tree by paper_2604_11920_b200.build); no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2604_11920_b200.build` "
+                          "(CUDA library for sm_100a; there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, f64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int
+    lib.tomo_lsqr_create.argtypes = [ctypes.POINTER(vp), i64, i64, i64, vp, vp, vp, ci, vp]
+    lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
+    lib.tomo_lsqr_solve_host.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
+    lib.tomo_lsqr_solve_multi.argtypes = [vp, i32, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
+    lib.tomo_lsqr_spmv.argtypes = [vp, ci, vp, vp, vp]
+    lib.tomo_lsqr_get_csc.argtypes = [vp, vp, vp, vp, vp]
+    lib.tomo_lsqr_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    lib.tomo_lsqr_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(f64)]
+    lib.tomo_lsqr_destroy.argtypes = [vp]
+    lib.tomo_lsqr_destroy.restype = None
+    lib.tomo_status_string.argtypes = [ci]
+    lib.tomo_status_string.restype = ctypes.c_char_p
+    for name in SYMBOLS:
+        if name not in ("tomo_lsqr_destroy", "tomo_status_string"):
+            getattr(lib, name).restype = ci
+    _lib = lib
+    return lib
+
+
+def _ptr(t) -> int | None:
+    """torch tensor / numpy array / int address / None -> address."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream) -> int | None:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    return getattr(stream, "cuda_stream", stream) or None
+
+
+def tomo_status_string(status: int) -> str:
+    return load().tomo_status_string(int(status)).decode()
+
+
+def tomo_lsqr_create(m, n, nnz, d_rowptr, d_colind, d_vals, vt=TOMO_VAL_F64, stream=None) -> int:
+    h = ctypes.c_void_p()
+    st = load().tomo_lsqr_create(ctypes.byref(h), m, n, nnz, _ptr(d_rowptr), _ptr(d_colind), _ptr(d_vals), vt, _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_create")
+    return h.value
+
+
+def tomo_lsqr_destroy(h) -> None:
+    if h:
+        load().tomo_lsqr_destroy(h)
+
+
+def tomo_lsqr_solve(h, d_b, damp, atol, btol, max_iters, d_x, h_r2norm_hist=None, h_arnorm_hist=None, stream=None) -> tomo_lsqr_result_t:
+    res = tomo_lsqr_result_t()
+    st = load().tomo_lsqr_solve(h, _ptr(d_b), damp, atol, btol, max_iters, _ptr(d_x), ctypes.byref(res),
+                                _ptr(h_r2norm_hist), _ptr(h_arnorm_hist), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_solve")
+    return res
+
+
+def tomo_lsqr_solve_host(h, h_b, damp, atol, btol, max_iters, h_x, stream=None) -> tomo_lsqr_result_t:
+    res = tomo_lsqr_result_t()
+    st = load().tomo_lsqr_solve_host(h, _ptr(h_b), damp, atol, btol, max_iters, _ptr(h_x), ctypes.byref(res), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_solve_host")
+    return res
+
+
+def tomo_lsqr_solve_multi(h, nrhs, d_B, damp, atol, btol, max_iters, d_X, stream=None):
+    res = (tomo_lsqr_result_t * nrhs)()
+    st = load().tomo_lsqr_solve_multi(h, nrhs, _ptr(d_B), damp, atol, btol, max_iters, _ptr(d_X), res, _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_solve_multi")
+    return list(res)
+
+
+def tomo_lsqr_spmv(h, transpose, d_in, d_out, stream=None) -> None:
+    st = load().tomo_lsqr_spmv(h, int(transpose), _ptr(d_in), _ptr(d_out), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_spmv")
+
+
+def tomo_lsqr_get_csc(h, d_colptr, d_rowind, d_cvals, stream=None) -> None:
+    st = load().tomo_lsqr_get_csc(h, _ptr(d_colptr), _ptr(d_rowind), _ptr(d_cvals), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_get_csc")
+
+
+def tomo_lsqr_set_option(h, key: str, value: int) -> None:
+    st = load().tomo_lsqr_set_option(h, key.encode(), int(value))
+    if st != TOMO_OK:
+        raise TomoError(st, f"tomo_lsqr_set_option({key})")
+
+
+def tomo_lsqr_get_info(h, key: str) -> float:
+    out = ctypes.c_double()
+    st = load().tomo_lsqr_get_info(h, key.encode(), ctypes.byref(out))
+    if st != TOMO_OK:
+        raise TomoError(st, f"tomo_lsqr_get_info({key})")
+    return out.value
+
+
+@dataclass
+class Result:
+    itn: int
+    istop: int
+    r1norm: float
+    r2norm: float
+    arnorm: float
+    anorm: float
+    acond: float
+    xnorm: float
+
+    @classmethod
+    def of(cls, r: tomo_lsqr_result_t) -> "Result":
+        return cls(r.itn, r.istop, r.r1norm, r.r2norm, r.arnorm, r.anorm, r.acond, r.xnorm)
+
+
+class TomoLsqr:
+    """Owns a handle and keeps the borrowed CSR device tensors alive (marshalling only)."""
+
+    def __init__(self, m, n, rowptr, colind, vals, stream=None):
+        import torch
+        assert rowptr.is_cuda and colind.is_cuda and vals.is_cuda
+        assert rowptr.dtype == torch.int64 and colind.dtype == torch.int32 and vals.dtype in (torch.float64, torch.float32)
+        self.m, self.n, self.nnz = int(m), int(n), int(colind.numel())
+        self._keep = (rowptr.contiguous(), colind.contiguous(), vals.contiguous())
+        vt = TOMO_VAL_F64 if vals.dtype == torch.float64 else TOMO_VAL_F32
+        self.h = tomo_lsqr_create(self.m, self.n, self.nnz, *self._keep, vt, stream)
+
+    def set(self, **opts):
+        for k, v in opts.items():
+            tomo_lsqr_set_option(self.h, k, v)
+        return self
+
+    def info(self, key):
+        return tomo_lsqr_get_info(self.h, key)
+
+    def spmv(self, x, transpose=False):
+        import torch
+        out = torch.empty(self.n if transpose else self.m, dtype=torch.float64, device=x.device)
+        tomo_lsqr_spmv(self.h, transpose, x, out)
+        return out
+
+    def csc(self):
+        import torch
+        dev = self._keep[0].device
+        colptr = torch.empty(self.n + 1, dtype=torch.int64, device=dev)
+        rowind = torch.empty(self.nnz, dtype=torch.int32, device=dev)
+        cvals = torch.empty(self.nnz, dtype=self._keep[2].dtype, device=dev)
+        tomo_lsqr_get_csc(self.h, colptr, rowind, cvals)
+        return colptr, rowind, cvals
+
+    def solve(self, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, history=False):
+        import numpy as np
+        import torch
+        x = torch.empty(self.n, dtype=torch.float64, device=b.device)
+        r2 = np.full(max(max_iters, 1), np.nan) if history else None
+        ar = np.full(max(max_iters, 1), np.nan) if history else None
+        res = Result.of(tomo_lsqr_solve(self.h, b, damp, atol, btol, max_iters, x, r2, ar))
+        if history:
+            return x, res, r2[: res.itn], ar[: res.itn]
+        return x, res
+
+    def solve_multi(self, B, damp=0.0, atol=0.0, btol=0.0, max_iters=50):
+        import torch
+        nrhs = B.shape[1]
+        X = torch.empty((self.n, nrhs), dtype=torch.float64, device=B.device)
+        res = tomo_lsqr_solve_multi(self.h, nrhs, B.contiguous(), damp, atol, btol, max_iters, X)
+        return X, [Result.of(r) for r in res]
+
+    def close(self):
+        if getattr(self, "h", None):
+            tomo_lsqr_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

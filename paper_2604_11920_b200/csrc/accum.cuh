@@ -1,0 +1,141 @@
+// accum.cuh — accumulators for the inner products of the LSQR hot path (device code only).
+//
+// Two accumulation modes (reading R-dd):
+//   MODE 0 "fast": fp64 FMA chains, several per lane, combined in a fixed order  -> deterministic,
+//                  within rounding of any other summation order.
+//   MODE 1 "dd"  : every product is formed exactly (TwoProd by FMA) and added into an unevaluated
+//                  double-double (hi, lo) (Knuth TwoSum); partial sums of lanes / warps / blocks are
+//                  combined by a dd+dd addition and the total is rounded to fp64 ONCE.  The rounded
+//                  result is the correctly rounded exact sum (up to ~1e-10-probability ties), hence
+//                  independent of the order of summation, which is what makes the fixed-k iterate
+//                  reproducible at scale.
+// This translation unit is compiled with --fmad=false: a fused multiply-add exists only where fma() is
+// written, so the error-free transformations below are not contracted away.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tomo {
+
+struct dd_t {
+  double hi, lo;
+};
+
+__device__ __forceinline__ void two_sum(double a, double b, double& s, double& t) {
+  s = a + b;
+  double bb = s - a;
+  t = (a - (s - bb)) + (b - bb);
+}
+
+__device__ __forceinline__ dd_t dd_add(dd_t a, dd_t b) {
+  double s, t;
+  two_sum(a.hi, b.hi, s, t);
+  t = t + (a.lo + b.lo);
+  dd_t r;
+  r.hi = s + t;
+  r.lo = t - (r.hi - s);
+  return r;
+}
+
+__device__ __forceinline__ double shfl_down_f64(double v, int off) { return __shfl_down_sync(0xffffffffu, v, off); }
+
+template <int MODE>
+struct Acc;
+
+template <>
+struct Acc<0> {
+  double s;
+  __device__ __forceinline__ void zero() { s = 0.0; }
+  __device__ __forceinline__ void mac(double a, double b) { s = fma(a, b, s); }
+  __device__ __forceinline__ void merge(const Acc& o) { s = s + o.s; }
+  __device__ __forceinline__ Acc down(int off) const {
+    Acc r;
+    r.s = shfl_down_f64(s, off);
+    return r;
+  }
+  __device__ __forceinline__ double value() const { return s; }
+  __device__ __forceinline__ double2 pack() const { return make_double2(s, 0.0); }
+  __device__ __forceinline__ void unpack(double2 p) { s = p.x; }
+};
+
+template <>
+struct Acc<1> {
+  dd_t v;
+  __device__ __forceinline__ void zero() { v.hi = 0.0; v.lo = 0.0; }
+  __device__ __forceinline__ void mac(double a, double b) {
+    double p = a * b;
+    double e = fma(a, b, -p);
+    double s, t;
+    two_sum(v.hi, p, s, t);
+    t = t + (v.lo + e);
+    v.hi = s + t;
+    v.lo = t - (v.hi - s);
+  }
+  __device__ __forceinline__ void merge(const Acc& o) { v = dd_add(v, o.v); }
+  __device__ __forceinline__ Acc down(int off) const {
+    Acc r;
+    r.v.hi = shfl_down_f64(v.hi, off);
+    r.v.lo = shfl_down_f64(v.lo, off);
+    return r;
+  }
+  __device__ __forceinline__ double value() const { return v.hi + v.lo; }
+  __device__ __forceinline__ double2 pack() const { return make_double2(v.hi, v.lo); }
+  __device__ __forceinline__ void unpack(double2 p) { v.hi = p.x; v.lo = p.y; }
+};
+
+// Sum over the lanes [base, base+WIDTH) of a warp, result valid in lane `base` (WIDTH = 32 or 8).
+template <int WIDTH, int MODE>
+__device__ __forceinline__ void lanes_reduce(Acc<MODE>& a) {
+#pragma unroll
+  for (int off = WIDTH / 2; off >= 1; off >>= 1) a.merge(a.down(off));
+}
+
+// Fixed-order block combine of one accumulator per warp (valid in lane 0 of each warp): result in
+// thread 0.  `slots` is shared memory for blockDim.x/32 double2.
+template <int MODE>
+__device__ __forceinline__ void block_combine(Acc<MODE>& a, double2* slots) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if (lane == 0) slots[warp] = a.pack();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a.unpack(slots[0]);
+    for (int w = 1; w < nw; ++w) {
+      Acc<MODE> o;
+      o.unpack(slots[w]);
+      a.merge(o);
+    }
+  }
+}
+
+// The last-arriving block of a launch sums the per-block partials in index order (bitwise
+// reproducible) and returns the total in thread 0.  Call with all threads of that block.
+template <int MODE>
+__device__ __forceinline__ double final_sum(const double2* partials, int count, double2* slots) {
+  Acc<MODE> a;
+  a.zero();
+  for (int i = threadIdx.x; i < count; i += blockDim.x) {
+    Acc<MODE> o;
+    o.unpack(__ldcg(partials + i));
+    a.merge(o);
+  }
+  lanes_reduce<32, MODE>(a);
+  __syncthreads();
+  block_combine<MODE>(a, slots);
+  return a.value();
+}
+
+// Publish this block's partial and find out whether it is the last block of the launch.
+__device__ __forceinline__ bool publish_and_ticket(double2* partials, double2 mine, unsigned int* ticket, int* s_flag) {
+  if (threadIdx.x == 0) {
+    __stcg(partials + blockIdx.x, mine);
+    __threadfence();
+    unsigned int t = atomicAdd(ticket, 1u);
+    *s_flag = (t == gridDim.x - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  bool last = (*s_flag != 0);
+  if (last) __threadfence();
+  return last;
+}
+
+}  // namespace tomo
