@@ -113,7 +113,9 @@ tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value
 
 /* Read-outs (host double): "create_ms", "transpose_ms", "csc_bytes", "scratch_bytes", "blocks_rows",
  * "blocks_cols", and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
- * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each). */
+ * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each);
+ * "kernels_enqueued": cumulative number of kernel launches this handle has issued in solves (nodes of
+ * replayed graphs included). */
 tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, double* out);
 
 void tomo_lsqr_destroy(tomo_lsqr_t h);

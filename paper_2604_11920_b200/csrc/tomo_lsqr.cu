@@ -71,6 +71,7 @@ struct tomo_lsqr_s {
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
+  double kernels_enqueued = 0;  // cumulative count of this library's kernel launches (graph nodes included)
   std::vector<cudaEvent_t> prof_ev;
 };
 
@@ -346,6 +347,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
   launch_spmv<OP_K2_INIT>(h, true, h->u, h->v, st);
   launch_vec<VOP_INIT_VW>(h, nullptr, h->v, h->w, nullptr, h->n, st);
   CK(cudaGetLastError());
+  h->kernels_enqueued += 3;
 
   const int k = h->check_every;
   const int chunks = max_iters > 0 ? (max_iters + k - 1) / k : 0;
@@ -374,6 +376,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
       }
       CK(cudaGetLastError());
     }
+    h->kernels_enqueued += 3.0 * k;
     // host poll: {itn, istop, stop}.  The next replay is enqueued before this one is inspected, so the
     // device never idles on the host; kernels after a stop return at once and leave x frozen.
     CK(cudaMemcpyAsync(&h->h_poll[slot], &h->sc->itn, sizeof(PollWord), cudaMemcpyDeviceToHost, st));
@@ -530,6 +533,7 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "k2_ms") *out = h->k2_ms;
   else if (k == "k4_ms") *out = h->k4_ms;
   else if (k == "k_launches") *out = h->k_launches;
+  else if (k == "kernels_enqueued") *out = h->kernels_enqueued;
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
 }

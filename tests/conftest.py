@@ -20,3 +20,10 @@ def cfg0():
     s = tomogen.System(0)
     rp, ci, va = s.csr()
     return dict(sys=s, m=s.dims.m, n=s.dims.n, rp=rp, ci=ci, va=va, b=s.rhs(0), damp=s.damp)
+
+
+def pytest_sessionfinish(session, exitstatus):
+    # stop the background oracle workers of the GPU parity tests (tests/oracle_jobs.py), if any
+    mod = sys.modules.get("oracle_jobs")
+    if mod is not None:
+        mod.shutdown()
