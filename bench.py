@@ -190,6 +190,10 @@ def run_ours(args) -> dict | None:
     x_host = torch.empty(n, dtype=torch.float64).pin_memory()
     S = tl.TomoLsqr(m, n, torch.from_numpy(rp).cuda(), torch.from_numpy(ci).cuda(), torch.from_numpy(va).cuda())
     S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0)
+    if args.engine is not None:
+        S.set(engine=args.engine)
+    if args.row_cost is not None:
+        S.set(row_cost=args.row_cost)
     b = b_host.cuda()
     x = torch.empty(n, dtype=torch.float64, device="cuda")
 
@@ -299,6 +303,8 @@ def main():
     ap.add_argument("--ref-iters", dest="ref_iters", type=int, default=20)
     ap.add_argument("--both-modes", dest="both_modes", action="store_true", default=True)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
+    ap.add_argument("--engine", type=int, default=None, help="tuning: SpMV kernel generation (library default if omitted)")
+    ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

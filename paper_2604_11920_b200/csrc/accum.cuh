@@ -62,14 +62,16 @@ template <>
 struct Acc<1> {
   dd_t v;
   __device__ __forceinline__ void zero() { v.hi = 0.0; v.lo = 0.0; }
+  // hi carries the fp64 running sum, lo the running sum of the exact rounding errors of every product
+  // (TwoProd by FMA) and every addition (Knuth TwoSum); (hi, lo) is not renormalised per term (the
+  // loop-carried dependency is one add on hi and one on lo), merge() and value() take it as it is.
   __device__ __forceinline__ void mac(double a, double b) {
     double p = a * b;
     double e = fma(a, b, -p);
-    double s, t;
-    two_sum(v.hi, p, s, t);
-    t = t + (v.lo + e);
-    v.hi = s + t;
-    v.lo = t - (v.hi - s);
+    double s, q;
+    two_sum(v.hi, p, s, q);
+    v.hi = s;
+    v.lo = v.lo + (q + e);
   }
   __device__ __forceinline__ void merge(const Acc& o) { v = dd_add(v, o.v); }
   __device__ __forceinline__ Acc down(int off) const {

@@ -15,6 +15,7 @@
 #include "../../include/tomo_lsqr.h"
 #include "build.cuh"
 #include "kernels.cuh"
+#include "stream.cuh"
 
 using namespace tomo;
 
@@ -55,8 +56,10 @@ struct tomo_lsqr_s {
   const int64_t* rowptr = nullptr; const int32_t* colind = nullptr; const void* vals = nullptr;
   // owned CSC (= CSR of A^T)
   int64_t* colptr = nullptr; int32_t* rowind = nullptr; void* cvals = nullptr;
-  // static partitions
+  // static partitions (row-group kernel) and element split points (stream kernel)
   int32_t* part_r = nullptr; int32_t* part_c = nullptr; int G = 0; bool part_dirty = true;
+  int64_t* sE_r = nullptr; int64_t* sE_c = nullptr; int32_t* sR_r = nullptr; int32_t* sR_c = nullptr;
+  CtaRec* cta_rec = nullptr; int SG = 0; int empty_rows = 0, empty_cols = 0;
   // work vectors and device state
   double *u = nullptr, *v = nullptr, *w = nullptr, *x = nullptr;
   Scalars* sc = nullptr; double2* part_spmv = nullptr; double2* part_vec = nullptr; int part_cap = 0;
@@ -67,7 +70,7 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, waves = 1;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, waves = 1, engine = 1, row_cost = 48;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
@@ -91,8 +94,44 @@ void launch_spmv_t(const tomo_lsqr_s* h, bool transpose, const double* x, double
   k_spmv<MODE, VT, OP><<<h->G, kThreads, 0, st>>>(ptr, idx, val, x, y, part, h->sc, h->part_spmv);
 }
 
+#ifndef TOMO_CH
+#define TOMO_CH 8192
+#endif
+#ifndef TOMO_W
+#define TOMO_W 16
+#endif
+#ifndef TOMO_S
+#define TOMO_S 2
+#endif
+using SCfg = StreamCfg<TOMO_CH, TOMO_W, TOMO_S>;
+
+template <int MODE, typename VT, int OP>
+void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  const int64_t* ptr = transpose ? h->colptr : h->rowptr;
+  const int32_t* idx = transpose ? h->rowind : h->colind;
+  const VT* val = (const VT*)(transpose ? h->cvals : h->vals);
+  const int nrows = (int)(transpose ? h->n : h->m);
+  auto kern = k_stream<SCfg, MODE, VT, OP>;
+  static bool attr_set = false;  // per instantiation
+  constexpr size_t smem = StreamSmem<SCfg, VT>::kTotal;
+  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+  kern<<<h->SG, SCfg::THREADS, smem, st>>>(ptr, idx, val, h->nnz, nrows, transpose ? h->empty_cols : h->empty_rows, x, y,
+                                           transpose ? h->sE_c : h->sE_r, transpose ? h->sR_c : h->sR_r, h->cta_rec, h->sc,
+                                           h->part_spmv);
+}
+
 template <int OP>
 void launch_spmv(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  if (h->engine == 1) {
+    if (h->vt == TOMO_VAL_F64) {
+      if (h->accumulate) launch_stream_t<1, double, OP>(h, transpose, x, y, st);
+      else launch_stream_t<0, double, OP>(h, transpose, x, y, st);
+    } else {
+      if (h->accumulate) launch_stream_t<1, float, OP>(h, transpose, x, y, st);
+      else launch_stream_t<0, float, OP>(h, transpose, x, y, st);
+    }
+    return;
+  }
   if (h->vt == TOMO_VAL_F64) {
     if (h->accumulate) launch_spmv_t<1, double, OP>(h, transpose, x, y, st);
     else launch_spmv_t<0, double, OP>(h, transpose, x, y, st);
@@ -133,6 +172,11 @@ tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
   k_partition_fix<<<1, 32, 0, st>>>(G, h->part_r);
   k_partition<<<gb, tb, 0, st>>>(h->colptr, h->n, G, kRowOverhead, kRowGroup, h->part_c);
   k_partition_fix<<<1, 32, 0, st>>>(G, h->part_c);
+  // stream kernel: one persistent CTA per SM, cost-balanced element split points
+  h->SG = h->sms;
+  const int gs = (h->SG + 1 + tb - 1) / tb;
+  k_stream_partition<<<gs, tb, 0, st>>>(h->rowptr, h->m, h->nnz, h->SG, h->row_cost, h->sE_r, h->sR_r);
+  k_stream_partition<<<gs, tb, 0, st>>>(h->colptr, h->n, h->nnz, h->SG, h->row_cost, h->sE_c, h->sR_c);
   CK(cudaGetLastError());
   h->part_dirty = false;
   return TOMO_OK;
@@ -189,6 +233,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
   cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
   cudaFree(h->part_r); cudaFree(h->part_c);
+  cudaFree(h->sE_r); cudaFree(h->sE_c); cudaFree(h->sR_r); cudaFree(h->sR_c); cudaFree(h->cta_rec);
   cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
   cudaFree(h->hist_r2); cudaFree(h->hist_ar); cudaFree(h->bh); cudaFree(h->xh);
@@ -251,6 +296,9 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
 #define ALLOC(p, bytes) if ((e = cudaMalloc(&(p), (bytes))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(work)"); break; }
     ALLOC(h->part_r, sizeof(int32_t) * h->part_cap);
     ALLOC(h->part_c, sizeof(int32_t) * h->part_cap);
+    ALLOC(h->sE_r, sizeof(int64_t) * (sms + 1)); ALLOC(h->sE_c, sizeof(int64_t) * (sms + 1));
+    ALLOC(h->sR_r, sizeof(int32_t) * (sms + 1)); ALLOC(h->sR_c, sizeof(int32_t) * (sms + 1));
+    ALLOC(h->cta_rec, sizeof(CtaRec) * sms);
     ALLOC(h->u, sizeof(double) * m); ALLOC(h->v, sizeof(double) * n);
     ALLOC(h->w, sizeof(double) * n); ALLOC(h->x, sizeof(double) * n);
     ALLOC(h->sc, sizeof(Scalars));
@@ -258,6 +306,19 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     ALLOC(h->part_vec, sizeof(double2) * h->part_cap);
 #undef ALLOC
     if ((e = cudaMemsetAsync(h->sc, 0, sizeof(Scalars), st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
+    {  // rows / columns without entries need the (rare) empty-row pass of the stream kernel
+      int* d_cnt = nullptr;
+      if ((e = cudaMalloc(&d_cnt, 2 * sizeof(int))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc"); break; }
+      cudaMemsetAsync(d_cnt, 0, 2 * sizeof(int), st);
+      k_count_empty<<<sms * 4, 256, 0, st>>>(h->rowptr, m, d_cnt);
+      k_count_empty<<<sms * 4, 256, 0, st>>>(h->colptr, n, d_cnt + 1);
+      int cnt[2] = {0, 0};
+      e = cudaMemcpyAsync(cnt, d_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      cudaFree(d_cnt);
+      if (e != cudaSuccess) { rc = cuda_fail(e, "count empty rows"); break; }
+      h->empty_rows = cnt[0]; h->empty_cols = cnt[1];
+    }
     if ((e = cudaMallocHost(&h->h_sc, sizeof(Scalars))) != cudaSuccess ||
         (e = cudaMallocHost(&h->h_poll, 2 * sizeof(PollWord))) != cudaSuccess) { rc = cuda_fail(e, "cudaMallocHost"); break; }
     for (int i = 0; i < 2; ++i)
@@ -296,7 +357,8 @@ void enqueue_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
 }
 
 tomo_status_t ensure_graph(tomo_lsqr_s* h) {
-  if (h->gexec && h->graph_k == h->check_every && h->graph_mode == h->accumulate && h->graph_G == h->G) return TOMO_OK;
+  const int gkey = h->accumulate + 2 * h->engine;
+  if (h->gexec && h->graph_k == h->check_every && h->graph_mode == gkey && h->graph_G == h->G) return TOMO_OK;
   if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   cudaGraph_t g = nullptr;
   CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
@@ -306,7 +368,7 @@ tomo_status_t ensure_graph(tomo_lsqr_s* h) {
   e = cudaGraphInstantiate(&h->gexec, g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-  h->graph_k = h->check_every; h->graph_mode = h->accumulate; h->graph_G = h->G;
+  h->graph_k = h->check_every; h->graph_mode = gkey; h->graph_G = h->G;
   return TOMO_OK;
 }
 
@@ -515,6 +577,8 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; if (h->accumulate != (int)value) h->part_dirty = true; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
+  else if (k == "engine") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->engine = (int)value; }
+  else if (k == "row_cost") { if (value < 0 || value > 4096) return TOMO_ERR_INVALID_ARG; if (h->row_cost != (int)value) h->part_dirty = true; h->row_cost = (int)value; }
   else if (k == "waves") { if (value < 1 || value > 16) return TOMO_ERR_INVALID_ARG; if (h->waves != (int)value) h->part_dirty = true; h->waves = (int)value; }
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
