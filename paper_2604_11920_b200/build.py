@@ -39,7 +39,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
-    tune = [f"-D{k}={os.environ[k]}" for k in ("TOMO_CH", "TOMO_W", "TOMO_S") if os.environ.get(k)]  # kernel-shape sweeps
+    tune = [f"-D{k}={os.environ[k]}" for k in ("TOMO_CH", "TOMO_W", "TOMO_S", "TOMO_PF") if os.environ.get(k)]  # kernel-shape sweeps
     cmd = [_nvcc()] + NVCC_FLAGS + tune + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True, cwd=CSRC)
     os.replace(LIB + ".tmp", LIB)

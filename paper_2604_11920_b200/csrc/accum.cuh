@@ -48,6 +48,11 @@ struct Acc<0> {
   __device__ __forceinline__ void zero() { s = 0.0; }
   __device__ __forceinline__ void mac(double a, double b) { s = fma(a, b, s); }
   __device__ __forceinline__ void merge(const Acc& o) { s = s + o.s; }
+  __device__ __forceinline__ void mac8(const double (&a)[8], const double (&b)[8]) {  // fixed tree
+    const double t0 = fma(a[1], b[1], a[0] * b[0]), t1 = fma(a[3], b[3], a[2] * b[2]);
+    const double t2 = fma(a[5], b[5], a[4] * b[4]), t3 = fma(a[7], b[7], a[6] * b[6]);
+    s = s + ((t0 + t1) + (t2 + t3));
+  }
   __device__ __forceinline__ Acc down(int off) const {
     Acc r;
     r.s = shfl_down_f64(s, off);
@@ -73,7 +78,30 @@ struct Acc<1> {
     v.hi = s;
     v.lo = v.lo + (q + e);
   }
-  __device__ __forceinline__ void merge(const Acc& o) { v = dd_add(v, o.v); }
+  __device__ __forceinline__ void merge(const Acc& o) {  // TwoSum of the his, errors collected in lo
+    double s, q;
+    two_sum(v.hi, o.v.hi, s, q);
+    v.hi = s;
+    v.lo = (v.lo + o.v.lo) + q;
+  }
+  // the products of eight (a, b) pairs at once: exact products (TwoProd), a TwoSum tree over them and
+  // one plain sum of all the rounding errors; same flop count as eight mac() calls, a third of the depth
+  __device__ __forceinline__ void mac8(const double (&a)[8], const double (&b)[8]) {
+    double p[8], e[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { p[u] = a[u] * b[u]; e[u] = fma(a[u], b[u], -p[u]); }
+    double s01, q01, s23, q23, s45, q45, s67, q67, s03, q03, s47, q47, s07, q07;
+    two_sum(p[0], p[1], s01, q01); two_sum(p[2], p[3], s23, q23);
+    two_sum(p[4], p[5], s45, q45); two_sum(p[6], p[7], s67, q67);
+    two_sum(s01, s23, s03, q03); two_sum(s45, s67, s47, q47);
+    two_sum(s03, s47, s07, q07);
+    const double err = ((((e[0] + e[1]) + (e[2] + e[3])) + ((e[4] + e[5]) + (e[6] + e[7]))) +
+                        ((q01 + q23) + (q45 + q67))) + ((q03 + q47) + q07);
+    double s, q;
+    two_sum(v.hi, s07, s, q);
+    v.hi = s;
+    v.lo = v.lo + (q + err);
+  }
   __device__ __forceinline__ Acc down(int off) const {
     Acc r;
     r.v.hi = shfl_down_f64(v.hi, off);

@@ -36,14 +36,15 @@
 namespace tomo {
 
 // ---- shapes -------------------------------------------------------------------------------------
-template <int CH_, int W_, int S_>
+template <int CH_, int W_, int S_, int PF_ = 4>
 struct StreamCfg {
+  static constexpr int PF = PF_;          // L2 prefetch distance in chunks (0: off)
   static constexpr int CH = CH_;          // elements per chunk (multiple of 32*W)
   static constexpr int W = W_;            // consumer warps
   static constexpr int S = S_;            // ring stages
   static constexpr int SL = CH_ / W_;     // elements per consumer slice
   static constexpr int MAXR = CH_ / 4;    // rows listed per chunk (a chunk is cut short beyond that)
-  static constexpr int THREADS = 32 * (W_ + 1);
+  static constexpr int THREADS = 32 * (W_ + 2);   // producer warp, resolver warp, W consumer warps
 };
 
 struct SliceRec {      // what a consumer leaves for the producer's chain, per slice and chunk
@@ -76,8 +77,8 @@ struct StreamSmem {
   static constexpr size_t kRs = sizeof(int32_t) * (CFG::MAXR + 8);
   static constexpr size_t kRec = sizeof(SliceRec) * CFG::W;
   static constexpr size_t kStage = ((kIdx + kVal + kRs + kRec + sizeof(StageHdr)) + 127) / 128 * 128;
-  static constexpr size_t kBars = 128;  // full[S], done[S]
-  static constexpr size_t kSlots = sizeof(double2) * (CFG::W + 1) + 16;
+  static constexpr size_t kBars = 256;  // full[S], done[S], freed[S]
+  static constexpr size_t kSlots = sizeof(double2) * (CFG::W + 2) + 16;
   static constexpr size_t kTotal = kStage * CFG::S + kBars + kSlots;
 };
 
@@ -116,6 +117,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                    smem_u32(dst)),
                "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
                : "memory");
+}
+
+// HBM -> L2 bulk prefetch (TMA engine, no shared memory): keeps the stream several chunks ahead of the ring
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 
 template <int MODE>
@@ -172,6 +178,174 @@ struct Chain {
   __device__ __forceinline__ void reset() { carry.zero(); carry_row = -1; carry_is_head = false; }
 };
 
+// The chain over records as a warp scan.  Lane l holds the record of slice (or CTA) l: an optional head
+// piece (state 1: its row continues, 2: its row ends here) followed by an optional tail piece (a row that
+// starts here and continues).  Each record is a map on the carry (partial sum and id of the open row):
+//   tail present -> carry := tail ;  head ends -> carry := none ;  else carry := carry + head
+// Maps compose associatively, so all carries come out of a 5-step Kogge-Stone scan in a fixed tree
+// order (deterministic) instead of a serial walk.  Returns, per lane, the row that ends in this record
+// (emit_row >= 0, or -2: the row that entered the CTA from the left) with its complete sum.
+template <int MODE>
+__device__ __forceinline__ void chain_scan(int hs, int ts, Acc<MODE> head, Acc<MODE> tail, int tail_row,
+                                           Acc<MODE>& carry, int& carry_row, bool& emit, Acc<MODE>& emit_sum,
+                                           int& emit_row) {
+  const int lane = threadIdx.x & 31;
+  int A = (ts || hs == 2) ? 0 : 1;
+  Acc<MODE> B;
+  B.zero();
+  if (ts) B = tail; else if (hs == 1) B = head;
+  int R = ts ? tail_row : -1;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int A1 = __shfl_up_sync(0xffffffffu, A, d);
+    const int R1 = __shfl_up_sync(0xffffffffu, R, d);
+    double2 bp = B.pack();
+    bp.x = __shfl_up_sync(0xffffffffu, bp.x, d);
+    bp.y = __shfl_up_sync(0xffffffffu, bp.y, d);
+    if (lane >= d && A) {  // own map keeps the carry: the earlier map's result flows through
+      Acc<MODE> B1 = acc_of<MODE>(bp);
+      B1.merge(B);
+      B = B1;
+      R = R1;
+      A = A1;
+    }
+  }
+  int Aex = __shfl_up_sync(0xffffffffu, A, 1);
+  int Rex = __shfl_up_sync(0xffffffffu, R, 1);
+  double2 bex = B.pack();
+  bex.x = __shfl_up_sync(0xffffffffu, bex.x, 1);
+  bex.y = __shfl_up_sync(0xffffffffu, bex.y, 1);
+  if (lane == 0) { Aex = 1; Rex = -1; bex = make_double2(0.0, 0.0); }
+  Acc<MODE> cin = acc_of<MODE>(bex);
+  int rin = Rex;
+  if (Aex) { Acc<MODE> t = carry; t.merge(cin); cin = t; rin = carry_row; }
+  emit = (hs == 2);
+  emit_sum = cin;
+  if (hs) emit_sum.merge(head);
+  emit_row = rin;
+  const int Al = __shfl_sync(0xffffffffu, A, 31), Rl = __shfl_sync(0xffffffffu, R, 31);
+  Acc<MODE> Bl = acc_bcast<MODE>(B, 31);
+  if (Al) { carry.merge(Bl); } else { carry = Bl; carry_row = Rl; }
+}
+
+// ---- consumer state of one slice sweep ---------------------------------------------------------------
+template <int MODE>
+struct Sweep {
+  Acc<MODE> acc;     // per-lane partial of the open row
+  double yold;       // lane 0: old y of the open row (fetched when the row starts inside the slice)
+  double2 h_val;     // lane 0: head record value
+  int cur;           // index of the open row in the chunk's row list (-1: the row open at the chunk start)
+  int next_b;        // chunk-local offset where the open row ends
+  int h_state;       // lane 0: head record state
+  bool started;      // the open row starts inside this slice
+  bool dirty;        // acc holds contributions
+};
+
+struct SweepCtx {    // uniform, read-only
+  const int32_t* rs; int nr; int r_first; int a; int b; int has_empty; double c; double sy; double* y;
+};
+
+// One 32-element step [base, base+32) of a slice that contains a row end (or starts at one): the lanes'
+// products v * x go to the rows they belong to; rows that end are reduced and finished (or recorded).
+// Shared by all unrolled steps of the sweep, hence not inlined.
+template <int MODE, int OP>
+__device__ __forceinline__ void sweep_slow_step(Sweep<MODE>& st, const SweepCtx& cx, Acc<MODE>& nsq, double v, double x,
+                                             int base) {
+  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
+  const int lane = threadIdx.x & 31;
+  const int32_t* rs = cx.rs;
+  const int hi = min(base + 32, cx.b);
+  const int pos = base + lane;
+  int lo = base;
+  while (true) {
+    if (!st.dirty && st.next_b < hi && st.cur + 2 <= cx.nr && rs[st.cur + 2] <= hi) {
+      // ---- segmented: two or more rows end inside [lo, hi) ----
+      const bool valid = pos >= lo && pos < hi;
+      int k = 0x7fffffff;
+      Acc<MODE> t;
+      t.zero();
+      if (!cx.has_empty) {  // starts of the following rows as a bit mask over the step
+        const int j = st.cur + 1 + lane;
+        const int sj = (j <= cx.nr) ? rs[j] : 0x7fffffff;
+        const unsigned bit = (sj < base + 32) ? (1u << (sj - base)) : 0u;
+        const unsigned M = __reduce_or_sync(0xffffffffu, bit);
+        if (valid) k = st.cur + __popc(M & ((2u << lane) - 1u));
+      } else if (valid) {
+        int l2 = st.cur + 1, h2 = cx.nr;
+        while (l2 < h2) { const int mid = (l2 + h2) >> 1; if (rs[mid] <= pos) l2 = mid + 1; else h2 = mid; }
+        k = l2 - 1;
+      }
+      if (valid) t.mac(v, x);
+      const int kprev = __shfl_up_sync(0xffffffffu, k, 1);
+      const bool head = valid && (pos == lo || kprev != k);
+      const int kend = valid ? rs[k + 1] : 0;
+      const bool fin = head && kend <= hi;
+      const bool fin_direct = fin && (k > st.cur || st.started);
+      double yo = 0.0;
+      if (NEEDS_Y && fin_direct) yo = cx.y[(int64_t)cx.r_first + k];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        Acc<MODE> o = t.down(d);
+        const int kk = __shfl_down_sync(0xffffffffu, k, d);
+        if (lane + d < 32 && kk == k) t.merge(o);
+      }
+      if (fin) {
+        if (fin_direct) finish_row_with<MODE, OP>(t, yo, cx.y, (int64_t)cx.r_first + k, cx.c, cx.sy, nsq);
+        else { st.h_val = t.pack(); st.h_state = 2; }
+      }
+      const int klast = __shfl_sync(0xffffffffu, k, hi - 1 - base);
+      const unsigned hb = __ballot_sync(0xffffffffu, head);
+      const int lhead = 31 - __clz((int)hb);
+      const int klast_end = rs[klast + 1];
+      if (klast_end > hi) {  // the last row of the step continues: it becomes the open row
+        Acc<MODE> hv = acc_bcast<MODE>(t, lhead);
+        st.acc.zero();
+        if (lane == 0) st.acc = hv;
+        st.dirty = true;
+        const bool newrow = klast > st.cur;
+        st.started = st.started || newrow;
+        st.cur = klast;
+        st.next_b = klast_end;
+        if (NEEDS_Y && newrow && lane == 0) st.yold = cx.y[(int64_t)cx.r_first + st.cur];
+      } else {
+        st.acc.zero();
+        st.dirty = false;
+        if (hi < cx.b) {
+          if (cx.has_empty) { int l2 = 0, h2 = cx.nr; while (l2 < h2) { const int mid = (l2 + h2) >> 1; if (rs[mid] <= hi) l2 = mid + 1; else h2 = mid; } st.cur = l2 - 1; }
+          else st.cur = klast + 1;
+          st.started = true;
+          st.next_b = rs[st.cur + 1];
+          if (NEEDS_Y && lane == 0) st.yold = cx.y[(int64_t)cx.r_first + st.cur];
+        } else st.next_b = hi;
+      }
+      return;
+    }
+    const int seg_end = min(st.next_b, hi);
+    if (lo < seg_end) {
+      const bool mine = pos >= lo && pos < seg_end;
+      st.acc.mac(mine ? v : 0.0, mine ? x : 0.0);  // other lanes add an exact zero
+      st.dirty = true;
+    }
+    if (st.next_b > hi) return;  // the open row continues behind the step
+    // the open row ends at next_b <= hi
+    lanes_reduce<32, MODE>(st.acc);
+    if (lane == 0) {
+      if (st.started) finish_row_with<MODE, OP>(st.acc, st.yold, cx.y, (int64_t)cx.r_first + st.cur, cx.c, cx.sy, nsq);
+      else { st.h_val = st.acc.pack(); st.h_state = 2; }
+    }
+    st.acc.zero();
+    st.dirty = false;
+    lo = st.next_b;
+    if (lo >= cx.b) return;  // slice finished exactly at a row end (next_b == b marks "nothing open")
+    if (cx.has_empty) { int l2 = 0, h2 = cx.nr; while (l2 < h2) { const int mid = (l2 + h2) >> 1; if (rs[mid] <= lo) l2 = mid + 1; else h2 = mid; } st.cur = l2 - 1; }
+    else st.cur = st.cur + 1;
+    st.started = true;
+    st.next_b = rs[st.cur + 1];
+    if (NEEDS_Y && lane == 0) st.yold = cx.y[(int64_t)cx.r_first + st.cur];
+    if (lo >= hi) return;
+  }
+}
+
 // ---- the kernel -----------------------------------------------------------------------------------
 // ptr/idx/val: CSR-like triple with `nrows` rows and `nnz` elements (K1: the CSR of A; K2: the CSC copy,
 // i.e. the CSR of A^T).  partE[b], partR[b] (b = 0..G): element split points (multiples of 4, partE[G] =
@@ -182,7 +356,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
          int nrows, int has_empty, const double* __restrict__ x, double* __restrict__ y,
          const int64_t* __restrict__ partE, const int32_t* __restrict__ partR, CtaRec* __restrict__ cta_rec, Scalars* sc,
          double2* partials) {
-  constexpr int CH = CFG::CH, W = CFG::W, S = CFG::S, SL = CFG::SL, MAXR = CFG::MAXR;
+  constexpr int CH = CFG::CH, W = CFG::W, S = CFG::S, SL = CFG::SL, MAXR = CFG::MAXR, PF = CFG::PF;
   using SM = StreamSmem<CFG, VT>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
 
@@ -207,12 +381,13 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   auto st_hdr = [&](int s) { return reinterpret_cast<StageHdr*>(stage_base(s) + SM::kIdx + SM::kVal + SM::kRs + SM::kRec); };
   uint64_t* bar_full = reinterpret_cast<uint64_t*>(smem_raw + SM::kStage * S);
   uint64_t* bar_done = bar_full + S;
+  uint64_t* bar_freed = bar_done + S;
   double2* s_slots = reinterpret_cast<double2*>(smem_raw + SM::kStage * S + SM::kBars);
-  int* s_flag = reinterpret_cast<int*>(s_slots + (W + 1));
+  int* s_flag = reinterpret_cast<int*>(s_slots + (W + 2));
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(bar_full + s, 1); mbar_init(bar_done + s, W); }
+    for (int s = 0; s < S; ++s) { mbar_init(bar_full + s, 1); mbar_init(bar_done + s, W); mbar_init(bar_freed + s, 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -225,85 +400,38 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   nsq.zero();
 
   if (warp == 0) {
-    // ============================== producer + chain ==============================
-    const uint64_t policy = l2_evict_first_policy();
-    Chain<MODE> ch;
-    ch.reset();
-    CtaRec my_rec;
-    my_rec.head = make_double2(0.0, 0.0); my_rec.tail = make_double2(0.0, 0.0);
-    my_rec.head_state = 0; my_rec.tail_state = 0; my_rec.tail_row = -1; my_rec.pad = 0;
-    int64_t e = E0;
-    int r = R0;
-    if (has_work && E0 < E1 && ptr[R0] > E0) {  // the range starts inside row R0-1
-      ch.carry_row = R0 - 1;
-      ch.carry_is_head = true;
-    }
-    int cidx = 0;           // chunks issued
-    int n_resolved = 0;     // chunks whose records have been chained
-    bool more = has_work;
-    // chain the records of the chunk in stage s; returns this lane's row to finish (or -1) and its sum
-    auto resolve = [&](int s, int& my_row, Acc<MODE>& my_sum) {
-      const SliceRec* rec = st_rec(s);
-      const int r_first = st_hdr(s)->r_first;
-      int n_emit = 0;
-      my_row = -1;
-      my_sum.zero();
-#pragma unroll 1
-      for (int w = 0; w < W; ++w) {
-        const int hs = rec[w].head_state, ts = rec[w].tail_state;
-        if (hs) {
-          ch.carry.merge(acc_of<MODE>(rec[w].head));
-          if (hs == 2) {
-            if (ch.carry_is_head) {
-              my_rec.head = ch.carry.pack();
-              my_rec.head_state = 2;
-            } else {
-              if (lane == n_emit) { my_row = ch.carry_row; my_sum = ch.carry; }
-              ++n_emit;
-            }
-            ch.reset();
-          }
-        }
-        if (ts) {
-          ch.carry = acc_of<MODE>(rec[w].tail);
-          ch.carry_row = r_first + rec[w].tail_k;
-          ch.carry_is_head = false;
-        }
-      }
-    };
-    constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
-    // rowptr entries of the next 32 rows, fetched one chunk ahead so that their latency overlaps the wait
-    int64_t pcur = (has_work && r + lane < R1) ? ptr[r + lane] : (int64_t)-1;
-    while (more || n_resolved < cidx) {
-      int my_row = -1;
-      Acc<MODE> my_sum;
-      my_sum.zero();
-      const int s = cidx % S;
-      if (more) {
-        if (cidx >= S) {  // the stage is still occupied by chunk cidx - S: wait for its consumers, chain it
-          mbar_wait(bar_done + s, ((cidx / S) - 1) & 1);
-          resolve(s, my_row, my_sum);
-          ++n_resolved;
-        }
-        // ---- describe chunk `cidx`: extent and the rows starting inside it ----
+    // ============================== producer: row lists + bulk copies ==============================
+    // Nothing in this loop waits on a global load issued in the same iteration: the row pointers of the
+    // next chunk are fetched one iteration ahead, the chain and the epilogues belong to warp 1.
+    if (has_work) {
+      const uint64_t policy = l2_evict_first_policy();
+      int64_t e = E0;
+      int r = R0;
+      int cidx = 0;
+      bool more = true;
+      // ptr[r + lane] for the next 32 rows (row R1 included: it delimits the last owned row)
+      int64_t pcur = (r + lane <= R1) ? ptr[r + lane] : (int64_t)-1;
+      while (more) {
+        const int s = cidx % S;
+        if (cidx >= S) mbar_wait(bar_freed + s, ((cidx / S) - 1) & 1);  // stage released by consumers and resolver
         int L = (int)min((int64_t)CH, E1 - e);
         const bool to_end = (e + L == E1);  // rows starting exactly at the range end belong to the next CTA, except trailing rows
         int32_t* rs = st_rs(s);
         int nr = 0;
         bool cut = false;
         int64_t p = pcur;
+        int64_t pnext = -1;
         while (true) {
           const int row = r + nr + lane;
           const bool in = (row < R1) && (p < e + L || to_end);
           const unsigned bal = __ballot_sync(0xffffffffu, in);
           if (in) rs[nr + lane] = (int)(p - e);
           const int cnt = __popc(bal);
+          if (cnt < 32) { pnext = __shfl_sync(0xffffffffu, p, cnt); nr += cnt; break; }  // lane cnt holds ptr[r + nr + cnt]
           nr += cnt;
-          if (cnt < 32) break;
-          if (nr >= MAXR) { cut = (r + nr < R1); break; }
-          p = (r + nr + lane < R1) ? ptr[r + nr + lane] : (int64_t)-1;
+          if (nr >= MAXR) { cut = (r + nr < R1); pnext = ptr[r + nr]; break; }
+          p = (r + nr + lane <= R1) ? ptr[r + nr + lane] : (int64_t)-1;
         }
-        int64_t pnext = ptr[r + nr];  // start of the first row not listed (r + nr <= nrows)
         if (cut && pnext < e + L) L = (int)(pnext - e);  // more than MAXR rows: the chunk ends where row r+nr starts
         const int64_t sent = pnext - e;
         const int skew = (int)(e & 3);
@@ -336,29 +464,73 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
           } else {
             mbar_arrive(bar_full + s);
           }
+          const int64_t pf0 = ((e + (int64_t)(PF - 1) * CH) + 3) & ~(int64_t)3;
+          const int64_t pf1 = min(pf0 + CH, E1 & ~(int64_t)3);
+          if (PF > 0 && pf1 > pf0) {
+            bulk_prefetch_l2(idx + pf0, (uint32_t)(pf1 - pf0) * 4u);
+            bulk_prefetch_l2(val + pf0, (uint32_t)(pf1 - pf0) * (uint32_t)sizeof(VT));
+          }
         }
         ++cidx;
-      } else {  // drain: chain the chunks still in the ring, oldest first
-        const int sd = n_resolved % S;
-        mbar_wait(bar_done + sd, (n_resolved / S) & 1);
-        resolve(sd, my_row, my_sum);
-        ++n_resolved;
+        pcur = (more && r + lane <= R1) ? ptr[r + lane] : (int64_t)-1;
       }
-      // both loads are issued before either is used: the row pointers of the next chunk and the old y
-      double yo = 0.0;
-      if (NEEDS_Y && my_row >= 0) yo = y[my_row];
-      pcur = (more && r + lane < R1) ? ptr[r + lane] : (int64_t)-1;
-      if (my_row >= 0) finish_row_with<MODE, OP>(my_sum, yo, y, my_row, c, sy, nsq);
     }
+  } else if (warp == 1) {
+    // ============================== resolver: chain of slice records + epilogues ==============================
+    Chain<MODE> ch;
+    ch.reset();
+    CtaRec my_rec;
+    my_rec.head = make_double2(0.0, 0.0); my_rec.tail = make_double2(0.0, 0.0);
+    my_rec.head_state = 0; my_rec.tail_state = 0; my_rec.tail_row = -1; my_rec.pad = 0;
+    Acc<MODE> carry;
+    carry.zero();
+    int carry_row = -1;  // -1: no open row; -2: the row that entered the range from the previous CTA
+    if (has_work && E0 < E1 && ptr[R0] > E0) carry_row = -2;
+    constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
+    int pend_row = -1;
+    Acc<MODE> pend_sum;
+    pend_sum.zero();
+    double pend_yo = 0.0;
+    int n = 0;
+    bool go = has_work;
+    while (go) {
+      const int s = n % S;
+      mbar_wait(bar_done + s, (n / S) & 1);
+      const SliceRec* rec = st_rec(s);
+      const int r_first = st_hdr(s)->r_first;
+      go = (st_hdr(s)->last == 0);
+      // lane w holds the record of slice w; the stage is handed back before anything slow happens
+      double2 l_head = make_double2(0.0, 0.0), l_tail = make_double2(0.0, 0.0);
+      int l_hs = 0, l_ts = 0, l_tk = 0;
+      if (lane < W) { l_head = rec[lane].head; l_tail = rec[lane].tail; l_hs = rec[lane].head_state; l_ts = rec[lane].tail_state; l_tk = rec[lane].tail_k; }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_freed + s);
+      bool emit;
+      Acc<MODE> e_sum;
+      int e_row;
+      chain_scan<MODE>(l_hs, l_ts, acc_of<MODE>(l_head), acc_of<MODE>(l_tail), r_first + l_tk, carry, carry_row, emit, e_sum, e_row);
+      // the row that entered the CTA from the left ends here: its sum goes to the CTA record
+      const unsigned hb = __ballot_sync(0xffffffffu, emit && e_row == -2);
+      if (hb) { const int src = __ffs((int)hb) - 1; my_rec.head = acc_bcast<MODE>(e_sum, src).pack(); my_rec.head_state = 2; }
+      // epilogue, one chunk behind: the old y of this chunk's rows is requested now and used next time
+      const int new_row = (emit && e_row >= 0) ? e_row : -1;
+      double new_yo = 0.0;
+      if (NEEDS_Y && new_row >= 0) new_yo = y[new_row];
+      if (pend_row >= 0) finish_row_with<MODE, OP>(pend_sum, pend_yo, y, pend_row, c, sy, nsq);
+      pend_row = new_row; pend_sum = e_sum; pend_yo = new_yo;
+      ++n;
+    }
+    if (pend_row >= 0) finish_row_with<MODE, OP>(pend_sum, pend_yo, y, pend_row, c, sy, nsq);
+    ch.carry = carry; ch.carry_row = carry_row; ch.carry_is_head = (carry_row == -2);
     // the row still open at the end of the range continues in the next CTA
-    if (ch.carry_row >= 0) {
+    if (ch.carry_row != -1) {
       if (ch.carry_is_head) { my_rec.head = ch.carry.pack(); my_rec.head_state = 1; }
       else { my_rec.tail = ch.carry.pack(); my_rec.tail_state = 1; my_rec.tail_row = ch.carry_row; }
     }
     if (lane == 0) cta_rec[blockIdx.x] = my_rec;
   } else if (has_work) {
     // ============================== consumers ==============================
-    const int w = warp - 1;
+    const int w = warp - 2;
     int cidx = 0;
     while (true) {
       const int s = cidx % S;
@@ -378,158 +550,115 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       int h_state = 0, t_state = 0, t_k = 0;
       double2 h_val = make_double2(0.0, 0.0), t_val = make_double2(0.0, 0.0);
       constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
+      constexpr int NSTEP = SL / 32;
       if (a < b) {
-        int q = a;
-        int cur = ub(a) - 1;                             // row containing element a (-1: open at the chunk start)
-        bool started = (cur >= 0) && (rs[cur] == a);      // ... and whether it starts exactly here
-        int next_b = rs[cur + 1];                         // where it ends
+        // ---- phase A: the slice's matrix entries to registers, all gathers of x in flight at once ----
+        double vv[NSTEP], xx[NSTEP];
+        {
+          int32_t cc[NSTEP];
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) {
+            const int p0 = a + 32 * u + lane;
+            const bool ok = p0 < b;
+            cc[u] = ok ? si[p0] : -1;
+            vv[u] = ok ? (double)sv[p0] : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) xx[u] = (cc[u] >= 0) ? __ldg(x + cc[u]) : 0.0;
+        }
+        // ---- phase B: sweep the steps; the row structure only decides where sums are closed ----
+        Sweep<MODE> st;
+        st.acc.zero();
+        st.dirty = false;
+        st.h_state = 0;
+        st.h_val = make_double2(0.0, 0.0);
+        st.cur = ub(a) - 1;                                      // row containing element a (-1: open at the chunk start)
+        st.started = (st.cur >= 0) && (rs[st.cur] == a);          // ... and whether it starts exactly here
+        st.next_b = rs[st.cur + 1];                               // where it ends
+        st.yold = 0.0;
+        SweepCtx cx;
+        cx.rs = rs; cx.nr = nr; cx.r_first = r_first; cx.a = a; cx.b = b; cx.has_empty = has_empty; cx.c = c; cx.sy = sy; cx.y = y;
         if (NEEDS_Y && nr > 2 * W) {  // many rows per slice: pull the old y of the slice's rows into L1
-          const int k0 = started ? cur : cur + 1;
+          const int k0 = st.started ? st.cur : st.cur + 1;
           const int64_t r0 = (int64_t)r_first + k0;
-          const int span = min(nr - k0, SL);  // at most SL rows can start inside the slice (without empty rows)
+          const int span = min(nr - k0, SL);
           for (int t = lane * 16; t < span; t += 32 * 16) prefetch_l1(y + r0 + t);
         }
-        Acc<MODE> acc;
-        acc.zero();
-        bool dirty = false;
-        double yold = 0.0;  // lane 0: old y of the open row, fetched when the row starts
-        if (NEEDS_Y && started && lane == 0) yold = y[(int64_t)r_first + cur];
-        while (q < b) {
-          const int qe = min(q + 32, b);
-          if (!dirty && next_b < qe && cur + 2 <= nr && rs[cur + 2] <= qe) {
-            // ---- segmented step: two or more rows end inside [q, qe) ----
-            const int pos = q + lane;
-            const bool valid = pos < qe;
-            int k = 0x7fffffff;
-            Acc<MODE> t;
-            t.zero();
-            if (!has_empty) {  // starts of the following rows as a bit mask over the step: k = cur + #starts <= pos
-              const int j = cur + 1 + lane;
-              const int sj = (j <= nr) ? rs[j] : 0x7fffffff;
-              const unsigned bit = (sj < q + 32) ? (1u << (sj - q)) : 0u;
-              const unsigned M = __reduce_or_sync(0xffffffffu, bit);
-              if (valid) k = cur + __popc(M & ((2u << lane) - 1u));
-            } else if (valid) {
-              int lo = cur + 1, hi = nr;  // rs[cur] <= q <= pos
-              while (lo < hi) { const int mid = (lo + hi) >> 1; if (rs[mid] <= pos) lo = mid + 1; else hi = mid; }
-              k = lo - 1;
-            }
-            if (valid) {
-              const int32_t col = si[pos];
-              double xv = __ldg(x + col);
-              if (SCALE_X) xv = xv * sx;
-              t.mac((double)sv[pos], xv);
-            }
-            const int kprev = __shfl_up_sync(0xffffffffu, k, 1);
-            const bool head = valid && (lane == 0 || kprev != k);
-            const int kend = valid ? rs[k + 1] : 0;
-            const bool fin = head && kend <= qe;            // the whole rest of row k is in this step
-            const bool fin_direct = fin && (k > cur || started);
-            double yo = 0.0;
-            if (NEEDS_Y && fin_direct) yo = y[(int64_t)r_first + k];
+        if (NEEDS_Y && st.started && lane == 0) st.yold = y[(int64_t)r_first + st.cur];
+        if (SCALE_X) {
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-              Acc<MODE> o = t.down(d);
-              const int kk = __shfl_down_sync(0xffffffffu, k, d);
-              if (lane + d < 32 && kk == k) t.merge(o);
-            }
-            if (fin) {
-              if (fin_direct) finish_row_with<MODE, OP>(t, yo, y, (int64_t)r_first + k, c, sy, nsq);
-              else { h_val = t.pack(); h_state = 2; }  // lane 0: the row open at the slice start ends here
-            }
-            const int nvalid = qe - q;
-            const int klast = __shfl_sync(0xffffffffu, k, nvalid - 1);
-            const unsigned hb = __ballot_sync(0xffffffffu, head);
-            const int lhead = 31 - __clz((int)hb);
-            const int klast_end = rs[klast + 1];
-            if (klast_end > qe) {  // the last row of the step continues: it becomes the open row
-              Acc<MODE> hv = acc_bcast<MODE>(t, lhead);
-              acc.zero();
-              if (lane == 0) acc = hv;
-              dirty = true;
-              const bool newrow = klast > cur;
-              started = started || newrow;
-              cur = klast;
-              next_b = klast_end;
-              if (NEEDS_Y && newrow && lane == 0) yold = y[(int64_t)r_first + cur];
-            } else {
-              acc.zero();
-              dirty = false;
-              if (qe < b) {
-                cur = has_empty ? ub(qe) - 1 : klast + 1;
-                started = true;
-                next_b = rs[cur + 1];
-                if (NEEDS_Y && lane == 0) yold = y[(int64_t)r_first + cur];
-              } else next_b = qe;
-            }
-            q = qe;
+          for (int u = 0; u < NSTEP; ++u) xx[u] = xx[u] * sx;
+        }
+        // Three shapes of a slice.  P0: it lies inside the open row (long rows: the common case).
+        // P1: exactly one row ends inside it and the next one runs on to the slice end or beyond.
+        // P2: anything else (short rows), step by step through one shared copy of the general code.
+        if (st.next_b >= b) {
+          if constexpr (NSTEP == 8) {
+            st.acc.mac8(vv, xx);
           } else {
-            // ---- plain steps: the rest of row `cur` inside the slice ----
-            const int seg_end = min(next_b, b);
-            for (; q + 256 <= seg_end; q += 256) {
-              const int p0 = q + lane;
-              int32_t cc[8];
-              double vv[8], xx[8];
 #pragma unroll
-              for (int u = 0; u < 8; ++u) { cc[u] = si[p0 + 32 * u]; vv[u] = (double)sv[p0 + 32 * u]; }
+            for (int u = 0; u < NSTEP; ++u) st.acc.mac(vv[u], xx[u]);
+          }
+          st.dirty = true;
+        } else if (!has_empty && rs[st.cur + 2] >= b) {
+          const int pe = st.next_b;  // a < pe < b
+          Acc<MODE> accB;
+          accB.zero();
+          double yold_new = 0.0;
+          if (NEEDS_Y && lane == 0) yold_new = y[(int64_t)r_first + st.cur + 1];
 #pragma unroll
-              for (int u = 0; u < 8; ++u) xx[u] = __ldg(x + cc[u]);
-#pragma unroll
-              for (int u = 0; u < 8; ++u) { if (SCALE_X) xx[u] = xx[u] * sx; acc.mac(vv[u], xx[u]); }
+          for (int u = 0; u < NSTEP; ++u) {
+            const int base = a + 32 * u;
+            if (base + 32 <= pe) st.acc.mac(vv[u], xx[u]);
+            else if (base >= pe) accB.mac(vv[u], xx[u]);
+            else {
+              const bool first = base + lane < pe;
+              st.acc.mac(first ? vv[u] : 0.0, first ? xx[u] : 0.0);
+              accB.mac(first ? 0.0 : vv[u], first ? 0.0 : xx[u]);
             }
-            if (q + 128 <= seg_end) {
-              const int p0 = q + lane;
-              const int32_t c0 = si[p0], c1 = si[p0 + 32], c2 = si[p0 + 64], c3 = si[p0 + 96];
-              const double v0 = (double)sv[p0], v1 = (double)sv[p0 + 32], v2 = (double)sv[p0 + 64], v3 = (double)sv[p0 + 96];
-              double x0 = __ldg(x + c0), x1 = __ldg(x + c1), x2 = __ldg(x + c2), x3 = __ldg(x + c3);
-              if (SCALE_X) { x0 = x0 * sx; x1 = x1 * sx; x2 = x2 * sx; x3 = x3 * sx; }
-              acc.mac(v0, x0); acc.mac(v1, x1); acc.mac(v2, x2); acc.mac(v3, x3);
-              q += 128;
-            }
-            {  // up to four more steps, the last one possibly partial: all gathers issued together
-              const int p0 = q + lane;
-              int32_t cc[4];
-              double vv[4], xx[4];
+          }
+          lanes_reduce<32, MODE>(st.acc);
+          if (lane == 0) {
+            if (st.started) finish_row_with<MODE, OP>(st.acc, st.yold, y, (int64_t)r_first + st.cur, c, sy, nsq);
+            else { st.h_val = st.acc.pack(); st.h_state = 2; }
+          }
+          st.acc = accB;
+          st.dirty = true;
+          st.cur = st.cur + 1;
+          st.started = true;
+          st.next_b = rs[st.cur + 1];
+          st.yold = yold_new;
+        } else {
+#pragma unroll 1
+          for (int u = 0; u < NSTEP; ++u) {
+            const int base = a + 32 * u;
+            if (base >= b) break;
+            const int p0 = base + lane;
+            const double vs = (p0 < b) ? (double)sv[p0] : 0.0;
+            double xs = xx[0];
 #pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const bool ok = p0 + 32 * u < seg_end;
-                cc[u] = ok ? si[p0 + 32 * u] : 0;
-                vv[u] = ok ? (double)sv[p0 + 32 * u] : 0.0;
-              }
-#pragma unroll
-              for (int u = 0; u < 4; ++u) xx[u] = (p0 + 32 * u < seg_end) ? __ldg(x + cc[u]) : 0.0;
-#pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                if (q + 32 * u < seg_end) {  // uniform
-                  if (SCALE_X) xx[u] = xx[u] * sx;
-                  acc.mac(vv[u], xx[u]);     // masked lanes add an exact zero
-                }
-              }
-              q = seg_end;
-            }
-            dirty = true;
-            if (q == next_b) {  // the row ends here
-              lanes_reduce<32, MODE>(acc);
-              if (lane == 0) {
-                if (started) finish_row_with<MODE, OP>(acc, yold, y, (int64_t)r_first + cur, c, sy, nsq);
-                else { h_val = acc.pack(); h_state = 2; }
-              }
-              acc.zero();
-              dirty = false;
-              if (q < b) {
-                cur = has_empty ? ub(q) - 1 : cur + 1;
-                started = true;
-                next_b = rs[cur + 1];
-                if (NEEDS_Y && lane == 0) yold = y[(int64_t)r_first + cur];
-              }
+            for (int k = 1; k < NSTEP; ++k) xs = (u == k) ? xx[k] : xs;
+            if (st.next_b >= base + 32 && base + 32 <= b) {  // the step lies inside the open row
+              st.acc.mac(vs, xs);
+              st.dirty = true;
+            } else {
+              sweep_slow_step<MODE, OP>(st, cx, nsq, vs, xs, base);
             }
           }
         }
-        if (next_b > b) {  // the open row continues behind the slice
-          lanes_reduce<32, MODE>(acc);
-          if (started) { t_val = acc.pack(); t_state = 1; t_k = cur; }
-          else { h_val = acc.pack(); h_state = 1; }
+        if (st.next_b == b && st.dirty) {  // the open row ends exactly at the slice end
+          lanes_reduce<32, MODE>(st.acc);
+          if (lane == 0) {
+            if (st.started) finish_row_with<MODE, OP>(st.acc, st.yold, y, (int64_t)r_first + st.cur, c, sy, nsq);
+            else { st.h_val = st.acc.pack(); st.h_state = 2; }
+          }
+        } else if (st.next_b > b) {  // the open row continues behind the slice
+          lanes_reduce<32, MODE>(st.acc);
+          if (st.started) { t_val = st.acc.pack(); t_state = 1; t_k = st.cur; }
+          else { st.h_val = st.acc.pack(); st.h_state = 1; }
         }
+        h_val = st.h_val;
+        h_state = st.h_state;
       }
       if (has_empty) {  // rows without elements: y_r = c * y_r
         const bool owns_end = (L == 0) ? (w == 0) : (a < L && L <= bfull);
@@ -566,7 +695,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   __syncthreads();
   if (threadIdx.x == 0) {
     Acc<MODE> tot = acc_of<MODE>(s_slots[0]);
-    for (int i = 1; i <= W; ++i) tot.merge(acc_of<MODE>(s_slots[i]));
+    for (int i = 1; i < W + 2; ++i) tot.merge(acc_of<MODE>(s_slots[i]));
     __stcg(partials + blockIdx.x, tot.pack());
     __threadfence();
     const unsigned int t = atomicAdd(&sc->ticket[0], 1u);
@@ -637,7 +766,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   __syncthreads();
   if (threadIdx.x == 0) {
     Acc<MODE> tot = acc_of<MODE>(s_slots[0]);
-    for (int i = 1; i <= W; ++i) tot.merge(acc_of<MODE>(s_slots[i]));
+    for (int i = 1; i < W + 2; ++i) tot.merge(acc_of<MODE>(s_slots[i]));
     const double total = tot.value();
     if (OP == OP_K1) tail_k1(sc, total);
     if (OP == OP_K2) tail_k2(sc, total);

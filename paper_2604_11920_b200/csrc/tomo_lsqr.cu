@@ -70,7 +70,7 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, waves = 1, engine = 1, row_cost = 48;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, waves = 1, engine = 1, row_cost = 96;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
@@ -95,15 +95,18 @@ void launch_spmv_t(const tomo_lsqr_s* h, bool transpose, const double* x, double
 }
 
 #ifndef TOMO_CH
-#define TOMO_CH 8192
+#define TOMO_CH 4096
 #endif
 #ifndef TOMO_W
 #define TOMO_W 16
 #endif
 #ifndef TOMO_S
-#define TOMO_S 2
+#define TOMO_S 3
 #endif
-using SCfg = StreamCfg<TOMO_CH, TOMO_W, TOMO_S>;
+#ifndef TOMO_PF
+#define TOMO_PF 0
+#endif
+using SCfg = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
 
 template <int MODE, typename VT, int OP>
 void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
