@@ -386,6 +386,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   int* s_flag = reinterpret_cast<int*>(s_slots + (W + 2));
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long t_start = clock64();
   if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) { mbar_init(bar_full + s, 1); mbar_init(bar_done + s, W); mbar_init(bar_freed + s, 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -527,6 +528,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       if (ch.carry_is_head) { my_rec.head = ch.carry.pack(); my_rec.head_state = 1; }
       else { my_rec.tail = ch.carry.pack(); my_rec.tail_state = 1; my_rec.tail_row = ch.carry_row; }
     }
+    my_rec.pad = (int)((clock64() - t_start) >> 4);  // busy time of this CTA in 16-cycle units (load-balance read-out)
     if (lane == 0) cta_rec[blockIdx.x] = my_rec;
   } else if (has_work) {
     // ============================== consumers ==============================
@@ -543,6 +545,10 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       const int a = w * SL, bfull = a + SL, b = min(bfull, L);
       // number of listed rows with start <= pos (uniform binary search in shared memory)
       auto ub = [&](int pos) {
+        if (nr <= 32) {  // the usual case (long rows): one shared-memory read and a vote
+          const int v = (lane < nr) ? rs[lane] : 0x7fffffff;
+          return __popc(__ballot_sync(0xffffffffu, v <= pos));
+        }
         int lo = 0, hi = nr;
         while (lo < hi) { const int mid = (lo + hi) >> 1; if (rs[mid] <= pos) lo = mid + 1; else hi = mid; }
         return lo;
@@ -554,7 +560,13 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       if (a < b) {
         // ---- phase A: the slice's matrix entries to registers, all gathers of x in flight at once ----
         double vv[NSTEP], xx[NSTEP];
-        {
+        if (b == bfull) {  // full slice (all but the last slices of a range): no predicates
+          int32_t cc[NSTEP];
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) { cc[u] = si[a + 32 * u + lane]; vv[u] = (double)sv[a + 32 * u + lane]; }
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) xx[u] = __ldg(x + cc[u]);
+        } else {
           int32_t cc[NSTEP];
 #pragma unroll
           for (int u = 0; u < NSTEP; ++u) {
@@ -595,6 +607,9 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
         if (st.next_b >= b) {
           if constexpr (NSTEP == 8) {
             st.acc.mac8(vv, xx);
+          } else if constexpr (NSTEP == 16) {
+            st.acc.mac8(*reinterpret_cast<const double(*)[8]>(&vv[0]), *reinterpret_cast<const double(*)[8]>(&xx[0]));
+            st.acc.mac8(*reinterpret_cast<const double(*)[8]>(&vv[8]), *reinterpret_cast<const double(*)[8]>(&xx[8]));
           } else {
 #pragma unroll
             for (int u = 0; u < NSTEP; ++u) st.acc.mac(vv[u], xx[u]);
@@ -708,47 +723,23 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
   Acc<MODE> extra;
   extra.zero();
   if (warp == 0) {
-    Chain<MODE> ch;
-    ch.reset();
     const int G = (int)gridDim.x;
-    int n_emit = 0, my_row = -1;
-    Acc<MODE> my_sum;
-    my_sum.zero();
-    for (int base = 0; base < G; base += 32) {
-      CtaRec rc;
-      rc.head_state = 0; rc.tail_state = 0; rc.tail_row = -1;
-      rc.head = make_double2(0.0, 0.0); rc.tail = make_double2(0.0, 0.0);
+    Acc<MODE> carry;
+    carry.zero();
+    int carry_row = -1;
+    for (int base = 0; base < G; base += 32) {  // 32 CTA records per scan
+      double2 hv = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
+      int hs = 0, ts = 0, trow = -1;
       if (base + lane < G) {
         const CtaRec* g = cta_rec + base + lane;
-        rc.head = __ldcg(&g->head); rc.tail = __ldcg(&g->tail);
-        rc.head_state = __ldcg(&g->head_state); rc.tail_state = __ldcg(&g->tail_state); rc.tail_row = __ldcg(&g->tail_row);
+        hv = __ldcg(&g->head); tv = __ldcg(&g->tail);
+        hs = __ldcg(&g->head_state); ts = __ldcg(&g->tail_state); trow = __ldcg(&g->tail_row);
       }
-      const int cntb = min(32, G - base);
-      for (int i = 0; i < cntb; ++i) {
-        const int hs = __shfl_sync(0xffffffffu, rc.head_state, i), ts = __shfl_sync(0xffffffffu, rc.tail_state, i);
-        if (hs) {
-          double2 hv;
-          hv.x = __shfl_sync(0xffffffffu, rc.head.x, i); hv.y = __shfl_sync(0xffffffffu, rc.head.y, i);
-          ch.carry.merge(acc_of<MODE>(hv));
-          if (hs == 2) {
-            if (ch.carry_row >= 0) {
-              if (lane == n_emit) { my_row = ch.carry_row; my_sum = ch.carry; }
-              ++n_emit;
-            }
-            ch.reset();
-          }
-        }
-        if (ts) {
-          double2 tv;
-          tv.x = __shfl_sync(0xffffffffu, rc.tail.x, i); tv.y = __shfl_sync(0xffffffffu, rc.tail.y, i);
-          ch.carry = acc_of<MODE>(tv);
-          ch.carry_row = __shfl_sync(0xffffffffu, rc.tail_row, i);
-        }
-        if (n_emit == 32 || (base + i == G - 1)) {
-          if (my_row >= 0) finish_row<MODE, OP>(my_sum, y, my_row, c, sy, extra);
-          n_emit = 0; my_row = -1;
-        }
-      }
+      bool emit;
+      Acc<MODE> e_sum;
+      int e_row;
+      chain_scan<MODE>(hs, ts, acc_of<MODE>(hv), acc_of<MODE>(tv), trow, carry, carry_row, emit, e_sum, e_row);
+      if (emit && e_row >= 0) finish_row<MODE, OP>(e_sum, y, e_row, c, sy, extra);
     }
     lanes_reduce<32, MODE>(extra);
   }

@@ -601,6 +601,14 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "k4_ms") *out = h->k4_ms;
   else if (k == "k_launches") *out = h->k_launches;
   else if (k == "kernels_enqueued") *out = h->kernels_enqueued;
+  else if (k == "cta_busy_min" || k == "cta_busy_max" || k == "cta_busy_mean") {
+    // busy cycles of the persistent CTAs in the most recent SpMV launch (load balance of the static split)
+    std::vector<CtaRec> rec(h->SG);
+    CK(cudaMemcpy(rec.data(), h->cta_rec, sizeof(CtaRec) * h->SG, cudaMemcpyDeviceToHost));
+    double mn = 1e300, mx = 0, sum = 0;
+    for (const CtaRec& r : rec) { const double c = 16.0 * (double)r.pad; mn = std::min(mn, c); mx = std::max(mx, c); sum += c; }
+    *out = k == "cta_busy_min" ? mn : k == "cta_busy_max" ? mx : sum / std::max(1, h->SG);
+  }
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
 }
