@@ -63,7 +63,7 @@ def ncu_traffic_bytes(config: int):
     try:
         for line in open(p):
             f = [t.strip() for t in line.split(",")]
-            if len(f) >= 3 and f[0] == f"cfg{config}" and f[1] == "k_spmv_mean_bytes_per_launch":
+            if len(f) >= 3 and f[0] == f"cfg{config}" and f[1] == "k_stream_mean_bytes_per_launch":
                 return float(f[2])
     except Exception:
         return None
@@ -128,6 +128,17 @@ def workload_name(s) -> str:
     d = s.dims
     return (f"configs[{s.config}]: {d.nx}x{d.ny}x{d.nz} grid, {d.m}x{d.n}, nnz {d.nnz}, damp {s.damp}, "
             f"atol=btol={s.solve['atol']:g}, max_iters {s.solve['max_iters']}")
+
+
+def aggregate_over_ranks(dist, ms: float, its: int, launches: float, device: str = "cuda"):
+    """Whole-job figures of N independent replicas: max over ranks of the device time, sums of the
+    iterations and launches (the only communication of the N > 1 path; gloo on CPU in the tests)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([float(its), launches], dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t[0]), int(c[0]), float(c[1])
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -218,11 +229,7 @@ def run_ours(args) -> dict | None:
         ms = e0.elapsed_time(e1)
         launches = S.info("kernels_enqueued") - k0
         if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            c = torch.tensor([float(its), launches], dtype=torch.float64, device="cuda")
-            dist.all_reduce(c, op=dist.ReduceOp.SUM)
-            ms, its, launches = float(t[0]), int(c[0]), float(c[1])
+            ms, its, launches = aggregate_over_ranks(dist, ms, its, launches, device="cuda")
         return ms, its, launches
 
     with ClockSampler(local) as clk:
@@ -270,8 +277,9 @@ def run_ours(args) -> dict | None:
                 "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "k_spmv (K1: A v - alpha u + norm; K2: A^T u - beta v + norm)",
+        "roofline": {"bound": "hbm", "kernel": "k_stream (K1: A v - alpha u + norm over CSR; K2: A^T u - beta v + norm over CSC), mean of the two launches of an iteration",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                     "algorithmic_bytes_per_launch": spmv_bytes / 2,
                      "peak_source": peak_src, "frac_of_8TBs": achieved / 8000.0,
                      "bytes_per_launch_pair": spmv_bytes, "k1_us": k1_us, "k2_us": k2_us, "k4_us": k4_us,
                      "k1_gbs": ab["k1"] / (k1_us * 1e-6) / 1e9, "k2_gbs": ab["k2"] / (k2_us * 1e-6) / 1e9},
