@@ -69,7 +69,7 @@ typedef struct {
 } tomo_lsqr_result_t;
 
 /* a0: validate the CSR arrays on the device, build the stable CSC transpose
- * (rows ascending inside each column) and the nnz-balanced row / column partitions.  One-off per matrix.
+ * (rows ascending inside each column) and the cost-balanced element split points of the persistent CTAs.  One-off per matrix.
  * vt selects the storage type of d_vals (arithmetic is fp64 either way). */
 tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr,
                                const int32_t* d_colind, const void* d_vals, tomo_valtype_t vt, void* cuda_stream);
@@ -108,14 +108,16 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *                          the order-independent iterate that parity at fixed k is claimed for)
  *   "graph"       0 | 1    replay a CUDA graph (default 1) or launch kernel by kernel
  *   "profile"     0 | 1    1: kernel-by-kernel launches bracketed by CUDA events (see tomo_lsqr_get_info)
- *   "waves"       w >= 1   static partitions per resident block slot (default 1) */
+ *   "row_cost"    c >= 0   weight of a row, in elements, in the cost-balanced element split of the
+ *                          persistent CTAs (default 96); changes the summation order only */
 tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value);
 
 /* Read-outs (host double): "create_ms", "transpose_ms", "csc_bytes", "scratch_bytes", "blocks_rows",
  * "blocks_cols", and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
  * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each);
  * "kernels_enqueued": cumulative number of kernel launches this handle has issued in solves (nodes of
- * replayed graphs included). */
+ * replayed graphs included); "cta_busy_min" / "cta_busy_mean" / "cta_busy_max": busy cycles of the persistent
+ * CTAs in the most recent sparse-product launch (load balance of the static split). */
 tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, double* out);
 
 void tomo_lsqr_destroy(tomo_lsqr_t h);

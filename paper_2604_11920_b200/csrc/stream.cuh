@@ -556,29 +556,9 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       int h_state = 0, t_state = 0, t_k = 0;
       double2 h_val = make_double2(0.0, 0.0), t_val = make_double2(0.0, 0.0);
       constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
-      constexpr int NSTEP = SL / 32;
+      constexpr int NSTEP = 8, SUB = 32 * NSTEP;  // a slice is swept in rounds of 256 elements
+      static_assert(SL % SUB == 0, "slice length must be a multiple of 256");
       if (a < b) {
-        // ---- phase A: the slice's matrix entries to registers, all gathers of x in flight at once ----
-        double vv[NSTEP], xx[NSTEP];
-        if (b == bfull) {  // full slice (all but the last slices of a range): no predicates
-          int32_t cc[NSTEP];
-#pragma unroll
-          for (int u = 0; u < NSTEP; ++u) { cc[u] = si[a + 32 * u + lane]; vv[u] = (double)sv[a + 32 * u + lane]; }
-#pragma unroll
-          for (int u = 0; u < NSTEP; ++u) xx[u] = __ldg(x + cc[u]);
-        } else {
-          int32_t cc[NSTEP];
-#pragma unroll
-          for (int u = 0; u < NSTEP; ++u) {
-            const int p0 = a + 32 * u + lane;
-            const bool ok = p0 < b;
-            cc[u] = ok ? si[p0] : -1;
-            vv[u] = ok ? (double)sv[p0] : 0.0;
-          }
-#pragma unroll
-          for (int u = 0; u < NSTEP; ++u) xx[u] = (cc[u] >= 0) ? __ldg(x + cc[u]) : 0.0;
-        }
-        // ---- phase B: sweep the steps; the row structure only decides where sums are closed ----
         Sweep<MODE> st;
         st.acc.zero();
         st.dirty = false;
@@ -597,6 +577,29 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
           for (int t = lane * 16; t < span; t += 32 * 16) prefetch_l1(y + r0 + t);
         }
         if (NEEDS_Y && st.started && lane == 0) st.yold = y[(int64_t)r_first + st.cur];
+#pragma unroll 1
+        for (int ar = a; ar < b; ar += SUB) {
+        const int br = min(ar + SUB, b);
+        // ---- phase A: the round's matrix entries to registers, all gathers of x in flight at once ----
+        double vv[NSTEP], xx[NSTEP];
+        if (br == ar + SUB) {  // full round: no predicates
+          int32_t cc[NSTEP];
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) { cc[u] = si[ar + 32 * u + lane]; vv[u] = (double)sv[ar + 32 * u + lane]; }
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) xx[u] = __ldg(x + cc[u]);
+        } else {
+          int32_t cc[NSTEP];
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) {
+            const int p0 = ar + 32 * u + lane;
+            const bool ok = p0 < br;
+            cc[u] = ok ? si[p0] : -1;
+            vv[u] = ok ? (double)sv[p0] : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < NSTEP; ++u) xx[u] = (cc[u] >= 0) ? __ldg(x + cc[u]) : 0.0;
+        }
         if (SCALE_X) {
 #pragma unroll
           for (int u = 0; u < NSTEP; ++u) xx[u] = xx[u] * sx;
@@ -604,26 +607,18 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
         // Three shapes of a slice.  P0: it lies inside the open row (long rows: the common case).
         // P1: exactly one row ends inside it and the next one runs on to the slice end or beyond.
         // P2: anything else (short rows), step by step through one shared copy of the general code.
-        if (st.next_b >= b) {
-          if constexpr (NSTEP == 8) {
-            st.acc.mac8(vv, xx);
-          } else if constexpr (NSTEP == 16) {
-            st.acc.mac8(*reinterpret_cast<const double(*)[8]>(&vv[0]), *reinterpret_cast<const double(*)[8]>(&xx[0]));
-            st.acc.mac8(*reinterpret_cast<const double(*)[8]>(&vv[8]), *reinterpret_cast<const double(*)[8]>(&xx[8]));
-          } else {
-#pragma unroll
-            for (int u = 0; u < NSTEP; ++u) st.acc.mac(vv[u], xx[u]);
-          }
+        if (st.next_b >= br) {
+          st.acc.mac8(vv, xx);
           st.dirty = true;
-        } else if (!has_empty && rs[st.cur + 2] >= b) {
-          const int pe = st.next_b;  // a < pe < b
+        } else if (!has_empty && rs[st.cur + 2] >= br) {
+          const int pe = st.next_b;  // ar <= pe < br
           Acc<MODE> accB;
           accB.zero();
           double yold_new = 0.0;
           if (NEEDS_Y && lane == 0) yold_new = y[(int64_t)r_first + st.cur + 1];
 #pragma unroll
           for (int u = 0; u < NSTEP; ++u) {
-            const int base = a + 32 * u;
+            const int base = ar + 32 * u;
             if (base + 32 <= pe) st.acc.mac(vv[u], xx[u]);
             else if (base >= pe) accB.mac(vv[u], xx[u]);
             else {
@@ -646,10 +641,10 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
         } else {
 #pragma unroll 1
           for (int u = 0; u < NSTEP; ++u) {
-            const int base = a + 32 * u;
-            if (base >= b) break;
+            const int base = ar + 32 * u;
+            if (base >= br) break;
             const int p0 = base + lane;
-            const double vs = (p0 < b) ? (double)sv[p0] : 0.0;
+            const double vs = (p0 < br) ? (double)sv[p0] : 0.0;
             double xs = xx[0];
 #pragma unroll
             for (int k = 1; k < NSTEP; ++k) xs = (u == k) ? xx[k] : xs;
@@ -661,6 +656,7 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
             }
           }
         }
+        }  // rounds
         if (st.next_b == b && st.dirty) {  // the open row ends exactly at the slice end
           lanes_reduce<32, MODE>(st.acc);
           if (lane == 0) {

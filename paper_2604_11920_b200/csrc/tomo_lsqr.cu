@@ -44,7 +44,6 @@ bool is_device_ptr(const void* p) {
 
 struct PollWord { int32_t itn, istop, stop; };
 
-constexpr int kRowOverhead = 16;     // per-row weight (in nnz) of the static partitions
 constexpr int kMaxProfileIters = 1 << 16;
 
 }  // namespace
@@ -56,8 +55,8 @@ struct tomo_lsqr_s {
   const int64_t* rowptr = nullptr; const int32_t* colind = nullptr; const void* vals = nullptr;
   // owned CSC (= CSR of A^T)
   int64_t* colptr = nullptr; int32_t* rowind = nullptr; void* cvals = nullptr;
-  // static partitions (row-group kernel) and element split points (stream kernel)
-  int32_t* part_r = nullptr; int32_t* part_c = nullptr; int G = 0; bool part_dirty = true;
+  // element split points of the persistent CTAs, per direction
+  bool part_dirty = true;
   int64_t* sE_r = nullptr; int64_t* sE_c = nullptr; int32_t* sR_r = nullptr; int32_t* sR_c = nullptr;
   CtaRec* cta_rec = nullptr; int SG = 0; int empty_rows = 0, empty_cols = 0;
   // work vectors and device state
@@ -70,7 +69,7 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, waves = 1, engine = 1, row_cost = 96;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 96;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
@@ -85,28 +84,19 @@ int vec_blocks(const tomo_lsqr_s* h, int64_t len) {
   return (int)std::max<int64_t>(1, std::min<int64_t>(b, (int64_t)h->sms * 8));
 }
 
-template <int MODE, typename VT, int OP>
-void launch_spmv_t(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
-  const int64_t* ptr = transpose ? h->colptr : h->rowptr;
-  const int32_t* idx = transpose ? h->rowind : h->colind;
-  const VT* val = (const VT*)(transpose ? h->cvals : h->vals);
-  const int32_t* part = transpose ? h->part_c : h->part_r;
-  k_spmv<MODE, VT, OP><<<h->G, kThreads, 0, st>>>(ptr, idx, val, x, y, part, h->sc, h->part_spmv);
-}
-
-#ifndef TOMO_CH
-#define TOMO_CH 4096
+// Kernel shapes <elements per chunk, consumer warps, ring stages, L2 prefetch distance>, per accumulation
+// mode (measured on B200, config 1): the double-double sums are instruction-bound, so they take the
+// longer slices (two 256-element rounds per slice, half the per-slice bookkeeping); the plain sums are
+// bandwidth-bound and take the deeper ring, which also leaves ~60 KB of L1 for the gathered vector.
+#ifdef TOMO_CH
+using SCfgFast = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
+using SCfgDD = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
+#else
+using SCfgFast = StreamCfg<4096, 16, 3, 0>;
+using SCfgDD = StreamCfg<8192, 16, 2, 0>;
 #endif
-#ifndef TOMO_W
-#define TOMO_W 16
-#endif
-#ifndef TOMO_S
-#define TOMO_S 3
-#endif
-#ifndef TOMO_PF
-#define TOMO_PF 0
-#endif
-using SCfg = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
+template <int MODE> struct SCfgOf { using type = SCfgFast; };
+template <> struct SCfgOf<1> { using type = SCfgDD; };
 
 template <int MODE, typename VT, int OP>
 void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
@@ -114,6 +104,7 @@ void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, doub
   const int32_t* idx = transpose ? h->rowind : h->colind;
   const VT* val = (const VT*)(transpose ? h->cvals : h->vals);
   const int nrows = (int)(transpose ? h->n : h->m);
+  using SCfg = typename SCfgOf<MODE>::type;
   auto kern = k_stream<SCfg, MODE, VT, OP>;
   static bool attr_set = false;  // per instantiation
   constexpr size_t smem = StreamSmem<SCfg, VT>::kTotal;
@@ -125,22 +116,12 @@ void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, doub
 
 template <int OP>
 void launch_spmv(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
-  if (h->engine == 1) {
-    if (h->vt == TOMO_VAL_F64) {
-      if (h->accumulate) launch_stream_t<1, double, OP>(h, transpose, x, y, st);
-      else launch_stream_t<0, double, OP>(h, transpose, x, y, st);
-    } else {
-      if (h->accumulate) launch_stream_t<1, float, OP>(h, transpose, x, y, st);
-      else launch_stream_t<0, float, OP>(h, transpose, x, y, st);
-    }
-    return;
-  }
   if (h->vt == TOMO_VAL_F64) {
-    if (h->accumulate) launch_spmv_t<1, double, OP>(h, transpose, x, y, st);
-    else launch_spmv_t<0, double, OP>(h, transpose, x, y, st);
+    if (h->accumulate) launch_stream_t<1, double, OP>(h, transpose, x, y, st);
+    else launch_stream_t<0, double, OP>(h, transpose, x, y, st);
   } else {
-    if (h->accumulate) launch_spmv_t<1, float, OP>(h, transpose, x, y, st);
-    else launch_spmv_t<0, float, OP>(h, transpose, x, y, st);
+    if (h->accumulate) launch_stream_t<1, float, OP>(h, transpose, x, y, st);
+    else launch_stream_t<0, float, OP>(h, transpose, x, y, st);
   }
 }
 
@@ -151,30 +132,9 @@ void launch_vec(const tomo_lsqr_s* h, const double* in0, double* a0, double* a1,
   else k_vec<0, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, len, h->sc, h->part_vec);
 }
 
-// resident blocks per SM of the heaviest SpMV instantiation for the current mode / value type
-int spmv_occupancy(const tomo_lsqr_s* h) {
-  int occ = 0;
-  cudaError_t e;
-  if (h->vt == TOMO_VAL_F64)
-    e = h->accumulate ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmv<1, double, OP_K2>, kThreads, 0)
-                      : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmv<0, double, OP_K2>, kThreads, 0);
-  else
-    e = h->accumulate ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmv<1, float, OP_K2>, kThreads, 0)
-                      : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_spmv<0, float, OP_K2>, kThreads, 0);
-  if (e != cudaSuccess) { cudaGetLastError(); occ = 2; }
-  return std::max(1, occ);
-}
-
 tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
   if (!h->part_dirty) return TOMO_OK;
-  int G = h->sms * spmv_occupancy(h) * h->waves;
-  G = std::min(G, h->part_cap - 1);
-  h->G = G;
-  const int tb = 128, gb = (G + 1 + tb - 1) / tb;
-  k_partition<<<gb, tb, 0, st>>>(h->rowptr, h->m, G, kRowOverhead, kRowGroup, h->part_r);
-  k_partition_fix<<<1, 32, 0, st>>>(G, h->part_r);
-  k_partition<<<gb, tb, 0, st>>>(h->colptr, h->n, G, kRowOverhead, kRowGroup, h->part_c);
-  k_partition_fix<<<1, 32, 0, st>>>(G, h->part_c);
+  const int tb = 128;
   // stream kernel: one persistent CTA per SM, cost-balanced element split points
   h->SG = h->sms;
   const int gs = (h->SG + 1 + tb - 1) / tb;
@@ -235,7 +195,6 @@ void free_handle(tomo_lsqr_s* h) {
   for (int i = 0; i < 2; ++i) if (h->ev_poll[i]) cudaEventDestroy(h->ev_poll[i]);
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
   cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
-  cudaFree(h->part_r); cudaFree(h->part_c);
   cudaFree(h->sE_r); cudaFree(h->sE_c); cudaFree(h->sR_r); cudaFree(h->sR_c); cudaFree(h->cta_rec);
   cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
@@ -297,8 +256,6 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     // --- work space ---
     h->part_cap = sms * 32 + 2;
 #define ALLOC(p, bytes) if ((e = cudaMalloc(&(p), (bytes))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(work)"); break; }
-    ALLOC(h->part_r, sizeof(int32_t) * h->part_cap);
-    ALLOC(h->part_c, sizeof(int32_t) * h->part_cap);
     ALLOC(h->sE_r, sizeof(int64_t) * (sms + 1)); ALLOC(h->sE_c, sizeof(int64_t) * (sms + 1));
     ALLOC(h->sR_r, sizeof(int32_t) * (sms + 1)); ALLOC(h->sR_c, sizeof(int32_t) * (sms + 1));
     ALLOC(h->cta_rec, sizeof(CtaRec) * sms);
@@ -360,8 +317,8 @@ void enqueue_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
 }
 
 tomo_status_t ensure_graph(tomo_lsqr_s* h) {
-  const int gkey = h->accumulate + 2 * h->engine;
-  if (h->gexec && h->graph_k == h->check_every && h->graph_mode == gkey && h->graph_G == h->G) return TOMO_OK;
+  const int gkey = h->accumulate;
+  if (h->gexec && h->graph_k == h->check_every && h->graph_mode == gkey && h->graph_G == h->SG) return TOMO_OK;
   if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   cudaGraph_t g = nullptr;
   CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
@@ -371,7 +328,7 @@ tomo_status_t ensure_graph(tomo_lsqr_s* h) {
   e = cudaGraphInstantiate(&h->gexec, g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) { h->gexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-  h->graph_k = h->check_every; h->graph_mode = gkey; h->graph_G = h->G;
+  h->graph_k = h->check_every; h->graph_mode = gkey; h->graph_G = h->SG;
   return TOMO_OK;
 }
 
@@ -580,9 +537,7 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; if (h->accumulate != (int)value) h->part_dirty = true; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
-  else if (k == "engine") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->engine = (int)value; }
   else if (k == "row_cost") { if (value < 0 || value > 4096) return TOMO_ERR_INVALID_ARG; if (h->row_cost != (int)value) h->part_dirty = true; h->row_cost = (int)value; }
-  else if (k == "waves") { if (value < 1 || value > 16) return TOMO_ERR_INVALID_ARG; if (h->waves != (int)value) h->part_dirty = true; h->waves = (int)value; }
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
 }
@@ -595,7 +550,7 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "transpose_ms") *out = h->transpose_ms;
   else if (k == "csc_bytes") *out = (double)h->nnz * (4.0 + vb) + 8.0 * (double)(h->n + 1);
   else if (k == "scratch_bytes") *out = h->scratch_bytes;
-  else if (k == "blocks_rows" || k == "blocks_cols") *out = (double)h->G;
+  else if (k == "blocks_rows" || k == "blocks_cols") *out = (double)h->SG;
   else if (k == "k1_ms") *out = h->k1_ms;
   else if (k == "k2_ms") *out = h->k2_ms;
   else if (k == "k4_ms") *out = h->k4_ms;

@@ -212,6 +212,49 @@ def test_fast_mode_reported_next_to_oracle_order_spread(big):
     g.S.set(accumulate=1)
 
 
+# ------------------------------------------------------------------------------- config 2, full size ---
+def test_config2_full_size_sampled_rows_and_properties(tl):
+    """BASELINE configs[2] (3 855 360 x 655 360, nnz 3.7e9, 45 GB CSR + 45 GB CSC on the device) in the
+    launch configuration bench.py --config 2 times.  The oracle cannot hold or sweep this system in
+    test time, so: A x on 3000 sampled rows against the oracle on exactly those rows (bitwise in dd mode);
+    A^T u for u supported on those rows against the oracle's scatter over them; the adjoint identity for
+    dense random vectors; 100 fixed iterations with a monotone residual and bitwise run-to-run
+    determinism.  (x_k against the dd oracle at k <= 20 was run once: DESIGN.md §11.)"""
+    free, total = torch.cuda.mem_get_info()
+    if total < 150e9:
+        pytest.skip("needs a 180 GB device")
+    s = tomogen.System(2)
+    d = s.dims
+    rp_d, ci_d, va_d = s.csr_cuda()
+    S = tl.TomoLsqr(d.m, d.n, rp_d, ci_d, va_d)
+    rng = np.random.default_rng(2)
+    xv, uv = rng.standard_normal(d.n), rng.standard_normal(d.m)
+    rows = np.sort(rng.choice(d.m, 3000, replace=False))
+    rows[-200:] = np.arange(d.m - 200, d.m)  # smoothing rows too
+    srp, sci, sva = s.rows(rows)
+    us = np.zeros(d.m)
+    us[rows] = rng.standard_normal(len(rows))
+    for acc in (1, 0):
+        S.set(accumulate=acc)
+        y = S.spmv(dev(xv)).cpu().numpy()
+        oy = oracle.spmv(len(rows), d.n, srp, sci, sva, xv, acc)
+        assert rel(y[rows], oy) <= TOL_SPMV and np.abs(y[rows] - oy).max() <= 1e-12 * np.abs(oy).max()
+        yt = S.spmv(dev(us), transpose=True).cpu().numpy()
+        oyt = oracle.spmv_t(len(rows), d.n, srp, sci, sva, us[rows], acc)
+        assert rel(yt, oyt) <= TOL_SPMV
+        if acc == 1:
+            assert np.array_equal(y[rows], oy) and np.array_equal(yt, oyt)
+        ytf = S.spmv(dev(uv), transpose=True).cpu().numpy()
+        assert abs(y @ uv - xv @ ytf) <= 1e-13 * np.linalg.norm(y) * np.linalg.norm(uv)
+    b = dev(s.rhs(0))
+    S.set(accumulate=1)
+    x1, res, r2, ar = S.solve(b, s.damp, 0.0, 0.0, 100, history=True)
+    assert (res.itn, res.istop) == (100, 7) and np.all(np.diff(r2) <= 1e-14 * r2[0])
+    x2, _ = S.solve(b, s.damp, 0.0, 0.0, 100)
+    assert torch.equal(x1, x2)
+    S.close()
+
+
 # ------------------------------------------------------------------------------- P7: fp32 values -------
 def test_fp32_values_path(tl, cfg0):
     va32 = cfg0["va"].astype(np.float32)

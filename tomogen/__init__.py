@@ -130,6 +130,37 @@ class System:
         self.fill(0, self.dims.m, ci, va)
         return rp, ci, va
 
+    def rows(self, rows) -> tuple:
+        """CSR (rowptr, colind, vals) of the sub-matrix made of the given rows (sampled-row checks at
+        sizes where the whole matrix is too big to hold twice)."""
+        rp = self.rowptr()
+        rows = np.asarray(rows, dtype=np.int64)
+        srp = np.zeros(len(rows) + 1, dtype=np.int64)
+        srp[1:] = np.cumsum(rp[rows + 1] - rp[rows])
+        ci = np.empty(int(srp[-1]), dtype=np.int32)
+        va = np.empty(int(srp[-1]), dtype=np.float64)
+        for k, r in enumerate(rows):
+            self.fill(int(r), int(r) + 1, ci[srp[k]:srp[k + 1]], va[srp[k]:srp[k + 1]])
+        return srp, ci, va
+
+    def csr_cuda(self, block_rows: int = 100000):
+        """The whole matrix as torch CUDA tensors (rowptr, colind, vals), generated and uploaded block by
+        block so that the host never holds more than one block (config 2: 45 GB of CSR)."""
+        import torch
+        rp = self.rowptr()
+        nnz = int(rp[-1])
+        ci_d = torch.empty(nnz, dtype=torch.int32, device="cuda")
+        va_d = torch.empty(nnz, dtype=torch.float64, device="cuda")
+        for r0 in range(0, self.dims.m, block_rows):
+            r1 = min(self.dims.m, r0 + block_rows)
+            e0, e1 = int(rp[r0]), int(rp[r1])
+            ci = np.empty(e1 - e0, dtype=np.int32)
+            va = np.empty(e1 - e0, dtype=np.float64)
+            self.fill(r0, r1, ci, va)
+            ci_d[e0:e1] = torch.from_numpy(ci).cuda()
+            va_d[e0:e1] = torch.from_numpy(va).cuda()
+        return torch.from_numpy(rp).cuda(), ci_d, va_d
+
     # --- vectors ----------------------------------------------------------------------------
     def x_true(self, rhs: int = 0) -> np.ndarray:
         x = np.empty(self.dims.n, dtype=np.float64)
