@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -556,6 +557,13 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "k4_ms") *out = h->k4_ms;
   else if (k == "k_launches") *out = h->k_launches;
   else if (k == "kernels_enqueued") *out = h->kernels_enqueued;
+  else if (k.rfind("cta_busy@", 0) == 0) {  // busy cycles of CTA <i> in the most recent sparse-product launch
+    const int i = atoi(k.c_str() + 9);
+    if (i < 0 || i >= h->SG) return TOMO_ERR_INVALID_ARG;
+    CtaRec r;
+    CK(cudaMemcpy(&r, h->cta_rec + i, sizeof(CtaRec), cudaMemcpyDeviceToHost));
+    *out = 16.0 * (double)r.pad;
+  }
   else if (k == "cta_busy_min" || k == "cta_busy_max" || k == "cta_busy_mean") {
     // busy cycles of the persistent CTAs in the most recent SpMV launch (load balance of the static split)
     std::vector<CtaRec> rec(h->SG);

@@ -128,6 +128,30 @@ def test_spmv_full_size(big):
         check_spmv(big[cfg][1], 5 + cfg)
 
 
+def test_spmv_random_structures(tl):
+    """Row-length mixes that hit every path of the streaming kernel: runs of empty rows (also at the very
+    beginning and end), rows of one entry, rows ending exactly on 32 / 256 / chunk boundaries, more short
+    rows per chunk than the row list holds, rows spanning several chunks and several CTAs."""
+    rng = np.random.default_rng(77)
+    cases = [
+        ("short", lambda: rng.integers(0, 9, size=60000)),
+        ("ones", lambda: np.ones(50000, dtype=np.int64)),
+        ("mostly_empty", lambda: np.where(rng.random(80000) < 0.02, rng.integers(1, 3000, size=80000), 0)),
+        ("aligned", lambda: rng.choice([32, 64, 256, 512, 4096, 8192], size=300)),
+        ("giant", lambda: np.array([0, 0, 700000, 0, 5, 300000, 0, 0, 0])),
+        ("mixed", lambda: np.concatenate([rng.integers(200, 2100, size=700), rng.integers(4, 8, size=20000), [0] * 500])),
+        ("tiny", lambda: np.array([3, 0, 1])),
+    ]
+    for name, make in cases:
+        lens = np.asarray(make(), dtype=np.int64)
+        n = int(max(lens.max(), 1) + rng.integers(0, 5000))
+        rp, ci, va = tomogen.random_csr(len(lens), n, lens, seed=int(rng.integers(1 << 30)))
+        g = Sys(tl, len(lens), n, rp, ci, va)
+        check_csc(g)
+        check_spmv(g, 100 + len(name))
+        g.S.close()
+
+
 def test_spmv_single_row_and_single_column(tl):
     rp, ci, va = tomogen.random_csr(1, 5000, [3000], seed=8)
     check_spmv(Sys(tl, 1, 5000, rp, ci, va), 9)
