@@ -723,19 +723,27 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
     Acc<MODE> carry;
     carry.zero();
     int carry_row = -1;
-    for (int base = 0; base < G; base += 32) {  // 32 CTA records per scan
-      double2 hv = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
-      int hs = 0, ts = 0, trow = -1;
+    // 32 CTA records per scan; the records of the next batch are requested before this one is scanned
+    auto load_rec = [&](int base, double2& hv, double2& tv, int& hs, int& ts, int& trow) {
+      hv = make_double2(0.0, 0.0); tv = make_double2(0.0, 0.0);
+      hs = 0; ts = 0; trow = -1;
       if (base + lane < G) {
         const CtaRec* g = cta_rec + base + lane;
         hv = __ldcg(&g->head); tv = __ldcg(&g->tail);
         hs = __ldcg(&g->head_state); ts = __ldcg(&g->tail_state); trow = __ldcg(&g->tail_row);
       }
+    };
+    double2 hv, tv, hv_n, tv_n;
+    int hs, ts, trow, hs_n, ts_n, trow_n;
+    load_rec(0, hv, tv, hs, ts, trow);
+    for (int base = 0; base < G; base += 32) {
+      load_rec(base + 32, hv_n, tv_n, hs_n, ts_n, trow_n);
       bool emit;
       Acc<MODE> e_sum;
       int e_row;
       chain_scan<MODE>(hs, ts, acc_of<MODE>(hv), acc_of<MODE>(tv), trow, carry, carry_row, emit, e_sum, e_row);
       if (emit && e_row >= 0) finish_row<MODE, OP>(e_sum, y, e_row, c, sy, extra);
+      hv = hv_n; tv = tv_n; hs = hs_n; ts = ts_n; trow = trow_n;
     }
     lanes_reduce<32, MODE>(extra);
   }

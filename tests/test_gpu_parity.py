@@ -293,6 +293,20 @@ def test_fp32_values_path(tl, cfg0):
     assert rel(x.cpu().numpy(), o64.x) <= TOL_F32
 
 
+def test_fp32_values_path_full_size(tl):
+    """R-f32 (i) at config-1 size: fp32 storage of the values (8 B per nonzero streamed), fp64 arithmetic;
+    against the dd oracle on the same rounded values x_50 agrees to 1e-8 (expected: bitwise)."""
+    s = tomogen.System(1)
+    rp_d, ci_d, va_d = s.csr_cuda()
+    S = tl.TomoLsqr(s.dims.m, s.dims.n, rp_d, ci_d, va_d.to(torch.float32))
+    del va_d
+    S.set(accumulate=1)
+    x, res = S.solve(dev(s.rhs(0)), s.damp, 0.0, 0.0, 50)
+    o = oracle_jobs.get("cfg1_dd_f32_50")
+    assert res.itn == 50 and rel(x.cpu().numpy(), o["x"]) <= TOL_X50
+    S.close()
+
+
 # ------------------------------------------------------------------------------- edge cases ------------
 def test_edge_cases(tl, g0, cfg0):
     m, n = g0.m, g0.n
