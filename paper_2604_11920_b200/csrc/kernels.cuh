@@ -51,7 +51,21 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
   } else {
     const double ra = sc->ralpha, t1 = sc->t1, t2 = sc->t2, rrho = sc->rrho;
     const bool norm_v = sc->norm_v != 0;
-    for (int64_t i = i0; i < len; i += stride) {
+    int64_t i = i0;
+    for (; i + 3 * stride < len; i += 4 * stride) {  // four independent elements per trip: 12 loads in flight
+      double v[4], w[4], xo[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { v[u] = a0[i + u * stride]; w[u] = a1[i + u * stride]; xo[u] = a2[i + u * stride]; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (norm_v) { v[u] = v[u] * ra; a0[i + u * stride] = v[u]; }
+        const double d = w[u] * rrho;
+        acc.mac(d, d);
+        a2[i + u * stride] = fma(t1, w[u], xo[u]);
+        a1[i + u * stride] = fma(t2, w[u], v[u]);
+      }
+    }
+    for (; i < len; i += stride) {
       double v = a0[i];
       if (norm_v) { v = v * ra; a0[i] = v; }
       double w = a1[i];

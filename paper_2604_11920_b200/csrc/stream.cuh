@@ -420,18 +420,40 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
         int32_t* rs = st_rs(s);
         int nr = 0;
         bool cut = false;
-        int64_t p = pcur;
+        // rows are taken 32 at a time from a window of rowptr entries; after the first block (fetched one
+        // chunk ahead) the window is refilled eight blocks at a time, so that a chunk full of short rows
+        // costs a few global round trips, not one per 32 rows
+        constexpr int NB = 8;
+        int64_t pw[NB];
+        pw[0] = pcur;
+        int have = 1;
         int64_t pnext = -1;
-        while (true) {
-          const int row = r + nr + lane;
-          const bool in = (row < R1) && (p < e + L || to_end);
-          const unsigned bal = __ballot_sync(0xffffffffu, in);
-          if (in) rs[nr + lane] = (int)(p - e);
-          const int cnt = __popc(bal);
-          if (cnt < 32) { pnext = __shfl_sync(0xffffffffu, p, cnt); nr += cnt; break; }  // lane cnt holds ptr[r + nr + cnt]
-          nr += cnt;
-          if (nr >= MAXR) { cut = (r + nr < R1); pnext = ptr[r + nr]; break; }
-          p = (r + nr + lane <= R1) ? ptr[r + nr + lane] : (int64_t)-1;
+        bool done = false;
+        while (!done) {
+#pragma unroll
+          for (int j = 0; j < NB; ++j) {
+            if (j < have && !done) {
+              const int64_t p = pw[j];
+              const int row = r + nr + lane;
+              const bool in = (row < R1) && (p < e + L || to_end);
+              const unsigned bal = __ballot_sync(0xffffffffu, in);
+              if (in) rs[nr + lane] = (int)(p - e);
+              const int cnt = __popc(bal);
+              if (cnt < 32) { pnext = __shfl_sync(0xffffffffu, p, cnt); nr += cnt; done = true; }  // lane cnt holds ptr[r + nr + cnt]
+              else {
+                nr += cnt;
+                if (nr >= MAXR) { cut = (r + nr < R1); pnext = ptr[r + nr]; done = true; }
+              }
+            }
+          }
+          if (!done) {
+#pragma unroll
+            for (int j = 0; j < NB; ++j) {
+              const int row = r + nr + 32 * j + lane;
+              pw[j] = (row <= R1) ? ptr[row] : (int64_t)-1;
+            }
+            have = NB;
+          }
         }
         if (cut && pnext < e + L) L = (int)(pnext - e);  // more than MAXR rows: the chunk ends where row r+nr starts
         const int64_t sent = pnext - e;

@@ -82,7 +82,7 @@ namespace {
 
 int vec_blocks(const tomo_lsqr_s* h, int64_t len) {
   int64_t b = (len + kThreads - 1) / kThreads;
-  return (int)std::max<int64_t>(1, std::min<int64_t>(b, (int64_t)h->sms * 8));
+  return (int)std::max<int64_t>(1, std::min<int64_t>(b, (int64_t)h->sms * 16));
 }
 
 // Kernel shapes <elements per chunk, consumer warps, ring stages, L2 prefetch distance>, per accumulation
@@ -255,7 +255,7 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     if (rc != TOMO_OK) break;
     cudaEventRecord(e2, st);
     // --- work space ---
-    h->part_cap = sms * 32 + 2;
+    h->part_cap = sms * 32 + 2;  // >= the largest grid of any kernel that publishes partials
 #define ALLOC(p, bytes) if ((e = cudaMalloc(&(p), (bytes))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(work)"); break; }
     ALLOC(h->sE_r, sizeof(int64_t) * (sms + 1)); ALLOC(h->sE_c, sizeof(int64_t) * (sms + 1));
     ALLOC(h->sR_r, sizeof(int32_t) * (sms + 1)); ALLOC(h->sR_c, sizeof(int32_t) * (sms + 1));
