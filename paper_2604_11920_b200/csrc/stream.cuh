@@ -421,9 +421,9 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
         int nr = 0;
         bool cut = false;
         // rows are taken 32 at a time from a window of rowptr entries; after the first block (fetched one
-        // chunk ahead) the window is refilled eight blocks at a time, so that a chunk full of short rows
+        // chunk ahead) the window is refilled two blocks at a time (more unrolling costs more in code size than it saves), so that a chunk full of short rows
         // costs a few global round trips, not one per 32 rows
-        constexpr int NB = 8;
+        constexpr int NB = 2;
         int64_t pw[NB];
         pw[0] = pcur;
         int have = 1;
