@@ -216,10 +216,29 @@ def run_ours(args) -> dict | None:
     b = b_host.cuda()
     x = torch.empty(n, dtype=torch.float64, device="cuda")
 
+    nrhs = s.dims.nrhs
+
+    class _Its:  # a step's iteration count (all right-hand sides)
+        def __init__(self, itn):
+            self.itn = itn
+
+    if nrhs > 1:  # configs[3]: the 8 right-hand sides (DESIGN.md a8: recurrences run one after the other)
+        B_host = torch.from_numpy(s.rhs_block()).pin_memory()
+        X_host = torch.empty((n, nrhs), dtype=torch.float64).pin_memory()
+        B = B_host.cuda()
+        X = torch.empty((n, nrhs), dtype=torch.float64, device="cuda")
+
     def step_device():
+        if nrhs > 1:
+            return _Its(sum(r.itn for r in tl.tomo_lsqr_solve_multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
         return tl.tomo_lsqr_solve(S.h, b, damp, atol, btol, max_iters, x)
 
     def step_host():
+        if nrhs > 1:  # no host-buffer entry for the block solve: copies around the device call
+            B.copy_(B_host, non_blocking=True)
+            r = _Its(sum(r.itn for r in tl.tomo_lsqr_solve_multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
+            X_host.copy_(X)
+            return r
         return tl.tomo_lsqr_solve_host(S.h, b_host, damp, atol, btol, max_iters, x_host)
 
     def timed(step):
@@ -277,11 +296,11 @@ def run_ours(args) -> dict | None:
         "data": "synthetic",
         "config": {"workload": workload_name(s), "iterations_per_step": its // max(1, args.steps * world),
                    "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
-                   "check_every": args.check_every, "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic", "parallelism": "replicas" if world > 1 else "single GPU",
+                   "check_every": args.check_every, "right_hand_sides": nrhs, "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic", "parallelism": "replicas" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {ab['iteration'] / 1e9:.2f} GB streamed per iteration vs 126 MB L2, no flush needed"},
         "effective_gbs": ab["iteration"] * its / world / (ms * 1e-3) / 1e9,
         "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms"),
-        "e2e": {"value": its_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * m, "d2h_bytes_per_step": 8 * n,
+        "e2e": {"value": its_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * m * nrhs, "d2h_bytes_per_step": 8 * n * nrhs,
                 "ms_per_step": ms_e2e / args.steps},
         "gpu_launches": int(launches),
         "clocks": clocks,

@@ -195,7 +195,7 @@ __device__ __forceinline__ void chain_scan(int hs, int ts, Acc<MODE> head, Acc<M
   B.zero();
   if (ts) B = tail; else if (hs == 1) B = head;
   int R = ts ? tail_row : -1;
-#pragma unroll
+#pragma unroll 1  // not on the critical path: keep the code small
   for (int d = 1; d < 32; d <<= 1) {
     const int A1 = __shfl_up_sync(0xffffffffu, A, d);
     const int R1 = __shfl_up_sync(0xffffffffu, R, d);
