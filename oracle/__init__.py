@@ -57,6 +57,8 @@ def _load():
         lib.oracle_lsqr_get_scalars.restype = None
         lib.oracle_lsqr_solve.argtypes = [i64, i64, vp, vp, vp, vp, f64, f64, f64, i32, ci, vp, vp, vp, vp, i32, vp, vp]
         lib.oracle_lsqr_solve.restype = None
+        lib.oracle_lsmr_solve.argtypes = lib.oracle_lsqr_solve.argtypes
+        lib.oracle_lsmr_solve.restype = None
         _lib = lib
     return _lib
 
@@ -130,6 +132,40 @@ def lsqr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=
     itn = int(res[0])
     return Result(x, itn, int(res[1]), res[2], res[3], res[4], res[5], res[6], res[7], r2h[:itn].copy(), arh[:itn].copy(),
                   {int(k): sx[i] for i, k in enumerate(snaps)})
+
+
+@dataclass
+class LsmrResult:
+    x: np.ndarray
+    itn: int
+    istop: int
+    normr: float
+    normar: float
+    normA: float
+    condA: float
+    normx: float
+    normr_hist: np.ndarray
+    normar_hist: np.ndarray
+    snapshots: dict
+
+
+def lsmr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, mode=PLAIN, snapshots=()):
+    """Run the oracle LSMR (Fong & Saunders; the paper's own solver)."""
+    rp, ci, va = _csr(rowptr, colind, vals)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    assert len(b) == m and len(rp) == m + 1
+    x = np.zeros(n, dtype=np.float64)
+    res = np.zeros(8, dtype=np.float64)
+    nrh = np.full(max(max_iters, 1), np.nan)
+    narh = np.full(max(max_iters, 1), np.nan)
+    snaps = np.ascontiguousarray(sorted(int(k) for k in snapshots), dtype=np.int32)
+    sx = np.full((len(snaps), n), np.nan)
+    _load().oracle_lsmr_solve(m, n, _p(rp), _p(ci), _p(va), _p(b), damp, atol, btol, int(max_iters), mode,
+                              _p(x), _p(res), _p(nrh), _p(narh), len(snaps), _p(snaps) if len(snaps) else None,
+                              _p(sx) if len(snaps) else None)
+    itn = int(res[0])
+    return LsmrResult(x, itn, int(res[1]), res[2], res[3], res[4], res[5], res[6], nrh[:itn].copy(), narh[:itn].copy(),
+                      {int(k): sx[i] for i, k in enumerate(snaps)})
 
 
 _SCALARS = ("itn", "istop", "alpha", "beta", "rhobar", "phibar", "bnorm", "anorm", "ddnorm", "res2", "xxnorm", "z",

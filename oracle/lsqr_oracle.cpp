@@ -229,6 +229,141 @@ struct Lsqr {
   }
 };
 
+
+// ---- LSMR (Fong & Saunders 2011): the solver the paper itself uses (ref. PAPER.md:249) ----
+// Same Golub-Kahan steps as LSQR; the solution is updated through h, hbar so that ||A^T r|| decreases
+// monotonically.  Step by step as published (damping by the extra rotation Qhat), inner products in the
+// same two accumulation modes; the vector updates are single fused multiply-adds.  NEXT-1 of SURVEY.md.
+
+// stable Givens rotation: [c s; -s c] [a; b] = [r; 0]
+inline void sym_ortho(double a, double b, double& c, double& s, double& r) {
+  if (b == 0.0) { c = (a > 0.0) - (a < 0.0); s = 0.0; r = std::fabs(a); }
+  else if (a == 0.0) { c = 0.0; s = (b > 0.0) - (b < 0.0); r = std::fabs(b); }
+  else if (std::fabs(b) > std::fabs(a)) {
+    double tau = a / b;
+    s = ((b > 0.0) ? 1.0 : -1.0) / std::sqrt(1.0 + tau * tau);
+    c = s * tau; r = b / s;
+  } else {
+    double tau = b / a;
+    c = ((a > 0.0) ? 1.0 : -1.0) / std::sqrt(1.0 + tau * tau);
+    s = c * tau; r = a / c;
+  }
+}
+
+struct Lsmr {
+  Csr A;
+  int mode;
+  double damp, atol, btol;
+  int32_t max_iters;
+  std::vector<double> u, v, h, hbar, x;
+  std::vector<dd> work;
+  double alpha = 0, beta = 0, normb = 0;
+  double zetabar = 0, alphabar = 0, rho = 1, rhobar = 1, cbar = 1, sbar = 0;
+  double betadd = 0, betad = 0, rhodold = 1, tautildeold = 0, thetatilde = 0, zeta = 0, d = 0;
+  double normA2 = 0, maxrbar = 0, minrbar = 1e100;
+  double normA = 0, condA = 1, normx = 0, normr = 0, normar = 0;
+  int32_t itn = 0, istop = 0;
+  bool done = false;
+
+  void init(const double* b) {
+    u.assign(b, b + A.m);
+    v.assign((size_t)A.n, 0.0); h.assign((size_t)A.n, 0.0); hbar.assign((size_t)A.n, 0.0); x.assign((size_t)A.n, 0.0);
+    beta = std::sqrt(sumsq(u.data(), A.m, mode));
+    normb = beta; normr = beta;
+    if (beta == 0.0) { done = true; istop = 0; return; }
+    double rb = 1.0 / beta;
+    for (int64_t i = 0; i < A.m; ++i) u[i] = u[i] * rb;
+    spmv_t(A, u.data(), 0.0, v.data(), mode, work);
+    alpha = std::sqrt(sumsq(v.data(), A.n, mode));
+    normar = alpha * beta;
+    if (alpha == 0.0) { done = true; istop = 0; return; }
+    double ra = 1.0 / alpha;
+    for (int64_t j = 0; j < A.n; ++j) v[j] = v[j] * ra;
+    h = v;
+    zetabar = alpha * beta; alphabar = alpha;
+    betadd = beta;
+    normA2 = alpha * alpha; normA = std::sqrt(normA2);
+    if (max_iters <= 0) { done = true; istop = 7; }
+  }
+
+  int32_t step() {
+    if (done) return istop;
+    ++itn;
+    spmv(A, v.data(), -alpha, u.data(), mode);
+    beta = std::sqrt(sumsq(u.data(), A.m, mode));
+    if (beta > 0.0) {
+      double rb = 1.0 / beta;
+      for (int64_t i = 0; i < A.m; ++i) u[i] = u[i] * rb;
+      spmv_t(A, u.data(), -beta, v.data(), mode, work);
+      alpha = std::sqrt(sumsq(v.data(), A.n, mode));
+      if (alpha > 0.0) {
+        double ra = 1.0 / alpha;
+        for (int64_t j = 0; j < A.n; ++j) v[j] = v[j] * ra;
+      }
+    }
+    // rotation Qhat for the damping term, then the rotations Q_k and Qbar_k
+    double chat, shat, alphahat;
+    sym_ortho(alphabar, damp, chat, shat, alphahat);
+    double rhoold = rho, c, s;
+    sym_ortho(alphahat, beta, c, s, rho);
+    double thetanew = s * alpha;
+    alphabar = c * alpha;
+    double rhobarold = rhobar, zetaold = zeta;
+    double thetabar = sbar * rho, rhotemp = cbar * rho;
+    sym_ortho(cbar * rho, thetanew, cbar, sbar, rhobar);
+    zeta = cbar * zetabar;
+    zetabar = -sbar * zetabar;
+    // hbar = h - (thetabar rho / (rhoold rhobarold)) hbar ;  x = x + (zeta / (rho rhobar)) hbar ;  h = v - (thetanew / rho) h
+    double f1 = -(thetabar * rho / (rhoold * rhobarold)), f2 = zeta / (rho * rhobar), f3 = -(thetanew / rho);
+    for (int64_t j = 0; j < A.n; ++j) {
+      double hb = std::fma(f1, hbar[j], h[j]);
+      hbar[j] = hb;
+      x[j] = std::fma(f2, hb, x[j]);
+      h[j] = std::fma(f3, h[j], v[j]);
+    }
+    // estimate of ||r||
+    double betaacute = chat * betadd, betacheck = -shat * betadd;
+    double betahat = c * betaacute;
+    betadd = -s * betaacute;
+    double thetatildeold = thetatilde, ctildeold, stildeold, rhotildeold;
+    sym_ortho(rhodold, thetabar, ctildeold, stildeold, rhotildeold);
+    thetatilde = stildeold * rhobar;
+    rhodold = ctildeold * rhobar;
+    betad = -stildeold * betad + ctildeold * betahat;
+    tautildeold = (zetaold - thetatildeold * tautildeold) / rhotildeold;
+    double taud = (zeta - thetatilde * tautildeold) / rhodold;
+    d = d + betacheck * betacheck;
+    normr = std::sqrt(d + (betad - taud) * (betad - taud) + betadd * betadd);
+    // estimates of ||A||, cond(A), ||A^T r||, ||x||
+    normA2 = normA2 + beta * beta;
+    normA = std::sqrt(normA2);
+    normA2 = normA2 + alpha * alpha;
+    maxrbar = std::fmax(maxrbar, rhobarold);
+    if (itn > 1) minrbar = std::fmin(minrbar, rhobarold);
+    condA = std::fmax(maxrbar, rhotemp) / std::fmin(minrbar, rhotemp);
+    normar = std::fabs(zetabar);
+    normx = std::sqrt(sumsq(x.data(), A.n, mode));
+    // stopping tests (conlim disabled)
+    double test1 = normr / normb;
+    double den2 = normA * normr;
+    double test2 = den2 > 0.0 ? normar / den2 : INFINITY;
+    double test3 = 1.0 / condA;
+    double ax = normA * normx / normb;
+    double tt1 = test1 / (1.0 + ax);
+    double rtol = btol + atol * ax;
+    istop = 0;
+    if (itn >= max_iters) istop = 7;
+    if (1.0 + test3 <= 1.0) istop = 6;
+    if (1.0 + test2 <= 1.0) istop = 5;
+    if (1.0 + tt1 <= 1.0) istop = 4;
+    if (test3 <= 0.0) istop = 3;
+    if (test2 <= atol) istop = 2;
+    if (test1 <= rtol) istop = 1;
+    if (istop != 0) done = true;
+    return istop;
+  }
+};
+
 }  // namespace
 
 extern "C" {
@@ -314,6 +449,32 @@ void oracle_lsqr_solve(int64_t m, int64_t n, const int64_t* rowptr, const int32_
   std::memcpy(x, s->x.data(), sizeof(double) * n);
   res[0] = s->itn; res[1] = s->istop; res[2] = s->r1norm; res[3] = s->r2norm; res[4] = s->arnorm;
   res[5] = s->anorm; res[6] = s->acond; res[7] = s->xnorm;
+  delete s;
+}
+
+// LSMR, whole solve.  res[0..7] = itn, istop, normr, normar, normA, condA, normx, 0.
+// nrhist / narhist: [max_iters] or NULL; snapshots as in oracle_lsqr_solve.
+void oracle_lsmr_solve(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
+                       const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
+                       double* x, double* res, double* nrhist, double* narhist,
+                       int32_t nsnap, const int32_t* snap_iters, double* snap_x) {
+  Lsmr* s = new Lsmr();
+  s->A = Csr{m, n, rowptr, colind, vals};
+  s->mode = mode; s->damp = damp; s->atol = atol; s->btol = btol; s->max_iters = max_iters;
+  s->init(b);
+  int32_t sn = 0;
+  while (!s->done) {
+    s->step();
+    if (nrhist) nrhist[s->itn - 1] = s->normr;
+    if (narhist) narhist[s->itn - 1] = s->normar;
+    while (sn < nsnap && snap_iters[sn] == s->itn) {
+      std::memcpy(snap_x + (int64_t)sn * n, s->x.data(), sizeof(double) * n);
+      ++sn;
+    }
+  }
+  std::memcpy(x, s->x.data(), sizeof(double) * n);
+  res[0] = s->itn; res[1] = s->istop; res[2] = s->normr; res[3] = s->normar; res[4] = s->normA;
+  res[5] = s->condA; res[6] = s->normx; res[7] = 0.0;
   delete s;
 }
 

@@ -8,21 +8,23 @@
 //   * One persistent CTA per SM.  CTA b owns the ELEMENT range [E_b, E_{b+1}) of the matrix arrays
 //     (cost-balanced split at multiples of 4 elements, not aligned to rows) and therefore streams one
 //     contiguous piece of `idx` and `val` from HBM exactly once.
-//   * Warp 0 is the producer: it cuts the range into chunks of <= CH elements, lists the rows that
-//     start inside each chunk (local offsets in shared memory), and moves the chunk's `idx` and `val`
-//     with two cp.async.bulk copies (TMA engine, L2 evict-first) into an S-stage shared-memory ring,
-//     completion signalled on an mbarrier.  S-1 chunks are always in flight: memory-level parallelism
-//     does not depend on registers or occupancy.
-//   * Warps 1..W are consumers: each sweeps a fixed slice of every chunk, 32 consecutive elements per
-//     step (conflict-free shared-memory reads), gathers x through L1/L2 and accumulates per-lane sums
-//     that are reduced once per row.  Rows that start and end inside a slice are finished by the
-//     consumer (axpy term, store, ||.||^2); pieces of rows that cross a slice boundary go to a small
-//     per-slice record, which the producer chains in slice order after the chunk is done
-//     (deterministic), finishing those rows.  Pieces of rows that cross a CTA boundary are chained by
-//     the last-arriving CTA of the launch, which also sums the per-CTA ||.||^2 partials in index order
-//     and runs the scalar step of the iteration (tails.cuh).
-//   * Short rows (two or more row ends inside one 32-element step, e.g. the 4-7 entry smoothing
-//     rows) take a segmented-reduction path: cost per step independent of the number of rows.
+//   * Warp 0, the producer, cuts the range into chunks of <= CH elements, lists the rows that start
+//     inside each chunk (local offsets in shared memory, row pointers fetched one chunk ahead) and moves
+//     the chunk's `idx` and `val` with two cp.async.bulk copies (TMA engine, L2 evict-first) into an
+//     S-stage shared-memory ring, completion signalled on an mbarrier.  Memory-level parallelism does
+//     not depend on registers or occupancy.
+//   * Warps 2..W+1 are consumers: each sweeps a fixed slice of every chunk in rounds of 256 elements.
+//     A round is first moved to registers (32 consecutive elements per load: conflict-free) with all
+//     eight gathers of x issued at once; then the products are added to a per-lane accumulator, and the
+//     row structure only decides where sums are closed (three shapes: inside one row / one row end /
+//     general, the last with a segmented warp reduction whose cost does not depend on the number of
+//     rows).  Rows that start and end inside a slice are finished by the consumer (axpy term, store,
+//     ||.||^2); pieces of rows that cross a slice boundary go to a small per-slice record.
+//   * Warp 1, the resolver, chains the records of a chunk with a log-step warp scan (fixed tree order:
+//     deterministic), hands the stage back to the producer and finishes the rows that ended, one chunk
+//     behind.  Pieces of rows that cross a CTA boundary are chained the same way by the last-arriving
+//     CTA of the launch, which also sums the per-CTA ||.||^2 partials in index order and runs the scalar
+//     step of the iteration (tails.cuh).
 // Every assignment (CTA ranges, chunks, slices, reduction trees) is static, so results are bitwise
 // reproducible in both accumulation modes.
 #pragma once
@@ -47,7 +49,7 @@ struct StreamCfg {
   static constexpr int THREADS = 32 * (W_ + 2);   // producer warp, resolver warp, W consumer warps
 };
 
-struct SliceRec {      // what a consumer leaves for the producer's chain, per slice and chunk
+struct SliceRec {      // what a consumer leaves for the resolver's chain, per slice and chunk
   double2 head;        // partial sum of the row that was open at the slice start
   double2 tail;        // partial sum of the row that started in the slice and continues behind it
   int head_state;      // 0 none, 1 row continues behind the slice, 2 row ended inside the slice
@@ -167,16 +169,6 @@ __device__ __forceinline__ void finish_row(Acc<MODE> sum, double* __restrict__ y
   finish_row_with<MODE, OP>(sum, yo, y, r, c, sy, nsq);
 }
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
-// The chain over slice (or CTA) records, executed uniformly by all lanes of a warp: rows whose last
-// piece has been seen are handed to lane `n_emit` for the global-memory epilogue.
-template <int MODE>
-struct Chain {
-  Acc<MODE> carry;
-  int carry_row;       // global row id of the open row, -1: none
-  bool carry_is_head;  // the open row started before this CTA: its sum belongs to the CTA record
-  __device__ __forceinline__ void reset() { carry.zero(); carry_row = -1; carry_is_head = false; }
-};
 
 // The chain over records as a warp scan.  Lane l holds the record of slice (or CTA) l: an optional head
 // piece (state 1: its row continues, 2: its row ends here) followed by an optional tail piece (a row that
@@ -500,8 +492,6 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
     }
   } else if (warp == 1) {
     // ============================== resolver: chain of slice records + epilogues ==============================
-    Chain<MODE> ch;
-    ch.reset();
     CtaRec my_rec;
     my_rec.head = make_double2(0.0, 0.0); my_rec.tail = make_double2(0.0, 0.0);
     my_rec.head_state = 0; my_rec.tail_state = 0; my_rec.tail_row = -1; my_rec.pad = 0;
@@ -544,11 +534,10 @@ k_stream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx, const
       ++n;
     }
     if (pend_row >= 0) finish_row_with<MODE, OP>(pend_sum, pend_yo, y, pend_row, c, sy, nsq);
-    ch.carry = carry; ch.carry_row = carry_row; ch.carry_is_head = (carry_row == -2);
     // the row still open at the end of the range continues in the next CTA
-    if (ch.carry_row != -1) {
-      if (ch.carry_is_head) { my_rec.head = ch.carry.pack(); my_rec.head_state = 1; }
-      else { my_rec.tail = ch.carry.pack(); my_rec.tail_state = 1; my_rec.tail_row = ch.carry_row; }
+    if (carry_row != -1) {
+      if (carry_row == -2) { my_rec.head = carry.pack(); my_rec.head_state = 1; }
+      else { my_rec.tail = carry.pack(); my_rec.tail_state = 1; my_rec.tail_row = carry_row; }
     }
     my_rec.pad = (int)((clock64() - t_start) >> 4);  // busy time of this CTA in 16-cycle units (load-balance read-out)
     if (lane == 0) cta_rec[blockIdx.x] = my_rec;
