@@ -82,6 +82,16 @@ tomo_status_t tomo_lsqr_solve(tomo_lsqr_t h, const double* d_b, double damp, dou
                               int32_t max_iters, double* d_x, tomo_lsqr_result_t* res, double* h_r2norm_hist,
                               double* h_arnorm_hist, void* cuda_stream);
 
+/* NEXT-1: the same problem by LSMR (Fong & Saunders 2011), the solver the paper itself uses
+ * (ref. P:249): identical bidiagonalisation kernels (A v, A^T u with fused norms), other scalar
+ * recurrences and a three-vector update (hbar, x, h), under which ||A^T r - damp^2 x|| decreases monotonically.
+ * Arguments as tomo_lsqr_solve.  Result fields: r2norm = sqrt(||b - A x||^2 + damp^2 ||x||^2) (estimate),
+ * arnorm = ||A^T r - damp^2 x|| (estimate), anorm, acond (estimates), xnorm = ||x|| (computed), r1norm from r2norm
+ * and xnorm; istop as above.  h_normr_hist / h_normar_hist: NULL or host fp64[max_iters]. */
+tomo_status_t tomo_lsmr_solve(tomo_lsqr_t h, const double* d_b, double damp, double atol, double btol,
+                              int32_t max_iters, double* d_x, tomo_lsqr_result_t* res, double* h_normr_hist,
+                              double* h_normar_hist, void* cuda_stream);
+
 /* The same solve with HOST buffers: h_b fp64[m] is copied to the device, h_x fp64[n] is copied back
  * (the end-to-end entry bench.py times; the matrix stays resident in the handle). */
 tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,

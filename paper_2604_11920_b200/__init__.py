@@ -22,7 +22,7 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
-    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsqr_solve_host", "tomo_lsqr_solve_multi", "tomo_lsqr_spmv",
+    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsqr_solve_multi", "tomo_lsqr_spmv",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
 )
 
@@ -54,6 +54,7 @@ def load() -> ctypes.CDLL:
     vp, i64, i32, f64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int
     lib.tomo_lsqr_create.argtypes = [ctypes.POINTER(vp), i64, i64, i64, vp, vp, vp, ci, vp]
     lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
+    lib.tomo_lsmr_solve.argtypes = lib.tomo_lsqr_solve.argtypes
     lib.tomo_lsqr_solve_host.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
     lib.tomo_lsqr_solve_multi.argtypes = [vp, i32, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
     lib.tomo_lsqr_spmv.argtypes = [vp, ci, vp, vp, vp]
@@ -112,6 +113,15 @@ def tomo_lsqr_solve(h, d_b, damp, atol, btol, max_iters, d_x, h_r2norm_hist=None
                                 _ptr(h_r2norm_hist), _ptr(h_arnorm_hist), _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_solve")
+    return res
+
+
+def tomo_lsmr_solve(h, d_b, damp, atol, btol, max_iters, d_x, h_normr_hist=None, h_normar_hist=None, stream=None) -> tomo_lsqr_result_t:
+    res = tomo_lsqr_result_t()
+    st = load().tomo_lsmr_solve(h, _ptr(d_b), damp, atol, btol, max_iters, _ptr(d_x), ctypes.byref(res),
+                                _ptr(h_normr_hist), _ptr(h_normar_hist), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsmr_solve")
     return res
 
 
@@ -208,13 +218,14 @@ class TomoLsqr:
         tomo_lsqr_get_csc(self.h, colptr, rowind, cvals)
         return colptr, rowind, cvals
 
-    def solve(self, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, history=False):
+    def solve(self, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, history=False, solver="lsqr"):
         import numpy as np
         import torch
         x = torch.empty(self.n, dtype=torch.float64, device=b.device)
         r2 = np.full(max(max_iters, 1), np.nan) if history else None
         ar = np.full(max(max_iters, 1), np.nan) if history else None
-        res = Result.of(tomo_lsqr_solve(self.h, b, damp, atol, btol, max_iters, x, r2, ar))
+        fn = {"lsqr": tomo_lsqr_solve, "lsmr": tomo_lsmr_solve}[solver]
+        res = Result.of(fn(self.h, b, damp, atol, btol, max_iters, x, r2, ar))
         if history:
             return x, res, r2[: res.itn], ar[: res.itn]
         return x, res

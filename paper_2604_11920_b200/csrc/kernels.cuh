@@ -25,8 +25,8 @@ constexpr int kWarps = kThreads / 32;
 //   VOP_K4     : v = v^ * (1/alpha) ; sum (w*rrho)^2 ; x += t1 w ; w = v + t2 w   (io0 = v, io1 = w, io2 = x)
 template <int MODE, int VOP>
 __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0, double* __restrict__ a0,
-                                                  double* __restrict__ a1, double* __restrict__ a2, int64_t len,
-                                                  Scalars* sc, double2* partials) {
+                                                  double* __restrict__ a1, double* __restrict__ a2,
+                                                  double* __restrict__ a3, int64_t len, Scalars* sc, double2* partials) {
   __shared__ double2 s_slots[kWarps];
   __shared__ int s_flag;
   if (VOP != VOP_INIT_U && sc->stop) return;
@@ -48,6 +48,20 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
       a1[i] = v;
     }
     return;
+  } else if (VOP == VOP_K4_LSMR) {  // a0 = v, a1 = h, a2 = x, a3 = hbar (Fong & Saunders' update)
+    const double ra = sc->ralpha, f1 = sc->f1, f2 = sc->f2, f3 = sc->f3;
+    const bool norm_v = sc->norm_v != 0;
+    for (int64_t i = i0; i < len; i += stride) {
+      double v = a0[i];
+      if (norm_v) { v = v * ra; a0[i] = v; }
+      const double h = a1[i];
+      const double hb = fma(f1, a3[i], h);
+      a3[i] = hb;
+      const double xn = fma(f2, hb, a2[i]);
+      a2[i] = xn;
+      a1[i] = fma(f3, h, v);
+      acc.mac(xn, xn);
+    }
   } else {
     const double ra = sc->ralpha, t1 = sc->t1, t2 = sc->t2, rrho = sc->rrho;
     const bool norm_v = sc->norm_v != 0;
@@ -82,6 +96,7 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
     if (threadIdx.x == 0) {
       if (VOP == VOP_INIT_U) tail_init_u(sc, total);
       if (VOP == VOP_K4) tail_k4(sc, total);
+      if (VOP == VOP_K4_LSMR) tail_k4_lsmr(sc, total);
       sc->ticket[1] = 0u;
     }
   }

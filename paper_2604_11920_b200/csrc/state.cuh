@@ -30,6 +30,14 @@ struct Scalars {
   int32_t beta_zero;       // beta_{k+1} == 0 in this iteration: the A^T pass is skipped
   int32_t norm_v;          // K4 must normalise v (alpha > 0 and the A^T pass ran)
   int32_t pad_;
+  // LSMR (solver = 1; Fong & Saunders 2011, the paper's own solver): same bidiagonalisation,
+  // other recurrences.  Results are reported through the fields above: r2norm = ||rbar||, arnorm = ||Abar^T rbar||,
+  // anorm = ||Abar|| estimate, acond, xnorm = ||x|| (computed, not estimated).
+  int32_t solver, pad2_;
+  double zetabar, alphabar, lrho, lrhobar, cbar, sbar;
+  double betadd, betad, rhodold, tautildeold, thetatilde, zeta, dsum;
+  double normA2, maxrbar, minrbar;
+  double f1, f2, f3;       // hbar = h + f1 hbar ; x = x + f2 hbar ; h = v + f3 h
   // last-block tickets, one per kernel kind (reset to 0 by the tail that consumed them)
   unsigned int ticket[4];
 };
@@ -45,7 +53,8 @@ enum SpmvOp : int {
 enum VecOp : int {
   VOP_INIT_U = 0,  // u^ = b, ||b||^2 ; tail: beta_1
   VOP_INIT_VW = 1, // v = v^/alpha, w = v, x = 0
-  VOP_K4 = 2       // v = v^/alpha ; ddnorm partial ; x += t1 w ; w = v + t2 w ; tail: stop tests
+  VOP_K4 = 2,      // v = v^/alpha ; ddnorm partial ; x += t1 w ; w = v + t2 w ; tail: stop tests
+  VOP_K4_LSMR = 3  // v = v^/alpha ; hbar = h + f1 hbar ; x += f2 hbar ; h = v + f3 h ; ||x||^2 ; tail: stop tests
 };
 
 }  // namespace tomo

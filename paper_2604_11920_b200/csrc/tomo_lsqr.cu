@@ -61,7 +61,8 @@ struct tomo_lsqr_s {
   int64_t* sE_r = nullptr; int64_t* sE_c = nullptr; int32_t* sR_r = nullptr; int32_t* sR_c = nullptr;
   CtaRec* cta_rec = nullptr; int SG = 0; int empty_rows = 0, empty_cols = 0;
   // work vectors and device state
-  double *u = nullptr, *v = nullptr, *w = nullptr, *x = nullptr;
+  double *u = nullptr, *v = nullptr, *w = nullptr, *x = nullptr, *hbar = nullptr;  // w doubles as LSMR's h
+  int solver = 0;  // 0 LSQR, 1 LSMR (set per solve)
   Scalars* sc = nullptr; double2* part_spmv = nullptr; double2* part_vec = nullptr; int part_cap = 0;
   double *hist_r2 = nullptr, *hist_ar = nullptr; int32_t hist_cap = 0;
   double *bh = nullptr, *xh = nullptr;   // device staging for solve_host
@@ -127,10 +128,17 @@ void launch_spmv(const tomo_lsqr_s* h, bool transpose, const double* x, double* 
 }
 
 template <int VOP>
-void launch_vec(const tomo_lsqr_s* h, const double* in0, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st) {
+void launch_vec(const tomo_lsqr_s* h, const double* in0, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st,
+                double* a3 = nullptr) {
   const int g = vec_blocks(h, len);
-  if (h->accumulate) k_vec<1, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, len, h->sc, h->part_vec);
-  else k_vec<0, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, len, h->sc, h->part_vec);
+  if (h->accumulate) k_vec<1, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
+  else k_vec<0, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
+}
+
+// the vector update that closes an iteration: LSQR's x / w step or LSMR's hbar / x / h step
+void launch_k4(const tomo_lsqr_s* h, cudaStream_t st) {
+  if (h->solver == 1) launch_vec<VOP_K4_LSMR>(h, nullptr, h->v, h->w, h->x, h->n, st, h->hbar);
+  else launch_vec<VOP_K4>(h, nullptr, h->v, h->w, h->x, h->n, st);
 }
 
 tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
@@ -197,7 +205,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
   cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
   cudaFree(h->sE_r); cudaFree(h->sE_c); cudaFree(h->sR_r); cudaFree(h->sR_c); cudaFree(h->cta_rec);
-  cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x);
+  cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x); cudaFree(h->hbar);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
   cudaFree(h->hist_r2); cudaFree(h->hist_ar); cudaFree(h->bh); cudaFree(h->xh);
   if (h->h_sc) cudaFreeHost(h->h_sc);
@@ -314,11 +322,11 @@ namespace {
 void enqueue_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
   launch_spmv<OP_K1>(h, false, h->v, h->u, st);
   launch_spmv<OP_K2>(h, true, h->u, h->v, st);
-  launch_vec<VOP_K4>(h, nullptr, h->v, h->w, h->x, h->n, st);
+  launch_k4(h, st);
 }
 
 tomo_status_t ensure_graph(tomo_lsqr_s* h) {
-  const int gkey = h->accumulate;
+  const int gkey = h->accumulate + 2 * h->solver;
   if (h->gexec && h->graph_k == h->check_every && h->graph_mode == gkey && h->graph_G == h->SG) return TOMO_OK;
   if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   cudaGraph_t g = nullptr;
@@ -350,6 +358,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
                            double* d_x, tomo_lsqr_result_t* res, double* h_r2, double* h_ar, cudaStream_t st) {
   const bool want_hist = (h_r2 || h_ar) && max_iters > 0;
   if (want_hist) { tomo_status_t rc = ensure_history(h, max_iters); if (rc != TOMO_OK) return rc; }
+  if (h->solver == 1 && !h->hbar) CK(cudaMalloc(&h->hbar, sizeof(double) * h->n));
   { tomo_status_t rc = rebuild_partitions(h, st); if (rc != TOMO_OK) return rc; }
   const bool profile = h->profile != 0;
   const bool graph = h->use_graph && !profile;
@@ -360,11 +369,13 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
   memset(hs, 0, sizeof(Scalars));
   hs->damp = damp; hs->atol = atol; hs->btol = btol; hs->max_iters = max_iters;
   hs->cs2 = -1.0;
+  hs->solver = h->solver;
   hs->hist_r2 = want_hist ? h->hist_r2 : nullptr;
   hs->hist_ar = want_hist ? h->hist_ar : nullptr;
   hs->hist_cap = want_hist ? h->hist_cap : 0;
   CK(cudaMemcpyAsync(h->sc, hs, sizeof(Scalars), cudaMemcpyHostToDevice, st));
   CK(cudaMemsetAsync(h->x, 0, sizeof(double) * h->n, st));
+  if (h->solver == 1) CK(cudaMemsetAsync(h->hbar, 0, sizeof(double) * h->n, st));
   // a1: beta_1 = ||b||, u^ = b, v^ = A^T u, alpha_1, w = v
   launch_vec<VOP_INIT_U>(h, d_b, h->u, nullptr, nullptr, h->m, st);
   launch_spmv<OP_K2_INIT>(h, true, h->u, h->v, st);
@@ -394,7 +405,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
         if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 1], st);
         launch_spmv<OP_K2>(h, true, h->u, h->v, st);
         if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 2], st);
-        launch_vec<VOP_K4>(h, nullptr, h->v, h->w, h->x, h->n, st);
+        launch_k4(h, st);
         if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 3], st);
       }
       CK(cudaGetLastError());
@@ -451,7 +462,21 @@ extern "C" tomo_status_t tomo_lsqr_solve(tomo_lsqr_t h, const double* d_b, doubl
   if (rc != TOMO_OK) return rc;
   if (!d_b || !d_x) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_b) || !is_device_ptr(d_x)) return TOMO_ERR_NOT_DEVICE_PTR;
+  h->solver = 0;
   return solve_device(h, d_b, damp, atol, btol, max_iters, d_x, res, h_r2norm_hist, h_arnorm_hist, (cudaStream_t)cuda_stream);
+}
+
+extern "C" tomo_status_t tomo_lsmr_solve(tomo_lsqr_t h, const double* d_b, double damp, double atol, double btol,
+                                         int32_t max_iters, double* d_x, tomo_lsqr_result_t* res, double* h_normr_hist,
+                                         double* h_normar_hist, void* cuda_stream) {
+  tomo_status_t rc = check_solve_args(h, damp, atol, btol, max_iters);
+  if (rc != TOMO_OK) return rc;
+  if (!d_b || !d_x) return TOMO_ERR_INVALID_ARG;
+  if (!is_device_ptr(d_b) || !is_device_ptr(d_x)) return TOMO_ERR_NOT_DEVICE_PTR;
+  h->solver = 1;
+  rc = solve_device(h, d_b, damp, atol, btol, max_iters, d_x, res, h_normr_hist, h_normar_hist, (cudaStream_t)cuda_stream);
+  h->solver = 0;
+  return rc;
 }
 
 extern "C" tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
@@ -463,6 +488,7 @@ extern "C" tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, 
   if (!h->bh) CK(cudaMalloc(&h->bh, sizeof(double) * h->m));
   if (!h->xh) CK(cudaMalloc(&h->xh, sizeof(double) * h->n));
   CK(cudaMemcpyAsync(h->bh, h_b, sizeof(double) * h->m, cudaMemcpyHostToDevice, st));
+  h->solver = 0;
   rc = solve_device(h, h->bh, damp, atol, btol, max_iters, h->xh, res, nullptr, nullptr, st);
   if (rc != TOMO_OK) return rc;
   CK(cudaMemcpyAsync(h_x, h->xh, sizeof(double) * h->n, cudaMemcpyDeviceToHost, st));
@@ -499,6 +525,7 @@ extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, cons
   if (!h->xh) CK(cudaMalloc(&h->xh, sizeof(double) * h->n));
   for (int r = 0; r < nrhs; ++r) {
     k_col_gather<<<vec_blocks(h, h->m), kThreads, 0, st>>>(d_B, nrhs, r, h->m, h->bh);
+    h->solver = 0;
     rc = solve_device(h, h->bh, damp, atol, btol, max_iters, h->xh, res ? res + r : nullptr, nullptr, nullptr, st);
     if (rc != TOMO_OK) return rc;
     k_col_scatter<<<vec_blocks(h, h->n), kThreads, 0, st>>>(h->xh, nrhs, r, h->n, d_X);

@@ -18,13 +18,17 @@ _jobs: dict[tuple, Future] = {}
 
 
 def _run(cfg: int, rhs: int, mode: int, damp: float, atol: float, btol: float, max_iters: int, snapshots: tuple,
-         f32_values: bool = False):
+         f32_values: bool = False, solver: str = "lsqr"):
     import oracle
     import tomogen
     s = tomogen.System(cfg)
     rp, ci, va = s.csr()
     if f32_values:  # the fp32-storage path: the oracle sees the same rounded values, widened to fp64
         va = va.astype(np.float32).astype(np.float64)
+    if solver == "lsmr":
+        r = oracle.lsmr(s.dims.m, s.dims.n, rp, ci, va, s.rhs(rhs), damp=damp, atol=atol, btol=btol, max_iters=max_iters,
+                        mode=mode, snapshots=snapshots)
+        return dict(x=r.x, itn=r.itn, istop=r.istop, snapshots=r.snapshots)
     b = s.rhs(rhs)
     r = oracle.lsqr(s.dims.m, s.dims.n, rp, ci, va, b, damp=damp, atol=atol, btol=btol, max_iters=max_iters,
                     mode=mode, snapshots=snapshots)
@@ -43,6 +47,8 @@ def _all_jobs():
         ("cfg1_plain_50",): (1, 0, oracle.PLAIN, d1, 0.0, 0.0, 50, (10,)),
         # config 1 with fp32-rounded values (DESIGN.md R-f32 (i))
         ("cfg1_dd_f32_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), True),
+        # config 1 by LSMR (NEXT-1)
+        ("cfg1_lsmr_dd_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), False, "lsmr"),
         # config 3: columns 0 and 7 of the 8 right-hand sides
         ("cfg3_dd_rhs0",): (3, 0, oracle.DD, d1, 0.0, 0.0, 50, ()),
         ("cfg3_dd_rhs7",): (3, 7, oracle.DD, d1, 0.0, 0.0, 50, ()),
@@ -55,7 +61,7 @@ def start():
     global _pool
     if _pool is not None:
         return
-    workers = max(1, min(6, (os.cpu_count() or 2) - 1))
+    workers = max(1, min(7, (os.cpu_count() or 2) - 1))
     _pool = ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn"))
     for key, args in _all_jobs().items():
         _jobs[key] = _pool.submit(_run, *args)

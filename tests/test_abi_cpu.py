@@ -21,7 +21,7 @@ def lib():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "tomo_lsqr.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(tomo_(?:lsqr|status)_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(tomo_(?:lsqr|lsmr|status)_[a-z_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported(lib):

@@ -279,6 +279,45 @@ def test_config2_full_size_sampled_rows_and_properties(tl):
     S.close()
 
 
+# ------------------------------------------------------------------------------- LSMR (NEXT-1) ---------
+def test_lsmr_cfg0_both_modes(g0, cfg0):
+    """tomo_lsmr_solve (the paper's own solver) against the LSMR oracle: x_50, iteration counts, both norm
+    histories, monotone ||A^T r||; bitwise in dd mode."""
+    b, damp = cfg0["b"], cfg0["damp"]
+    for acc in (0, 1):
+        g0.S.set(accumulate=acc)
+        x, res, nr, nar = g0.S.solve(dev(b), damp, 0.0, 0.0, 50, history=True, solver="lsmr")
+        o = oracle.lsmr(g0.m, g0.n, g0.rp, g0.ci, g0.va, b, damp=damp, max_iters=50, mode=acc)
+        assert rel(x.cpu().numpy(), o.x) <= TOL_X50 and (res.itn, res.istop) == (o.itn, o.istop) == (50, 7)
+        assert rel(nr, o.normr_hist) <= 1e-10 and rel(nar, o.normar_hist) <= 1e-8
+        assert np.all(np.diff(nar) <= 1e-12 * nar[0])
+        for mine, ref in ((res.r2norm, o.normr), (res.arnorm, o.normar), (res.anorm, o.normA), (res.acond, o.condA), (res.xnorm, o.normx)):
+            assert abs(mine - ref) <= 1e-9 * abs(ref)
+        if acc == 1:
+            assert np.array_equal(x.cpu().numpy(), o.x) and np.array_equal(nr, o.normr_hist)
+    # tolerance stop: same iteration and reason as the oracle; LSQR still works on the same handle afterwards
+    g0.S.set(accumulate=1)
+    x, res = g0.S.solve(dev(b), damp, 1e-6, 1e-6, 500, solver="lsmr")
+    o = oracle.lsmr(g0.m, g0.n, g0.rp, g0.ci, g0.va, b, damp=damp, atol=1e-6, btol=1e-6, max_iters=500, mode=oracle.DD)
+    assert (res.itn, res.istop) == (o.itn, o.istop) and rel(x.cpu().numpy(), o.x) <= TOL_X50
+    x2, res2 = g0.S.solve(dev(b), damp, 0.0, 0.0, 50)
+    o2 = oracle.lsqr(g0.m, g0.n, g0.rp, g0.ci, g0.va, b, damp=damp, max_iters=50, mode=oracle.DD)
+    assert np.array_equal(x2.cpu().numpy(), o2.x)
+    # b = 0 and max_iters = 0
+    x, res = g0.S.solve(torch.zeros(g0.m, dtype=torch.float64, device="cuda"), damp, 0.0, 0.0, 5, solver="lsmr")
+    assert res.itn == 0 and res.istop == 0 and not x.any()
+    x, res = g0.S.solve(dev(b), damp, 0.0, 0.0, 0, solver="lsmr")
+    assert res.itn == 0 and res.istop == 7 and not x.any()
+
+
+def test_lsmr_x50_cfg1(big):
+    s, g = big[1]
+    o = oracle_jobs.get("cfg1_lsmr_dd_50")
+    g.S.set(accumulate=1, check_every=10, graph=1)
+    x, res = g.S.solve(dev(s.rhs(0)), s.damp, 0.0, 0.0, 50, solver="lsmr")
+    assert res.itn == 50 and rel(x.cpu().numpy(), o["x"]) <= TOL_X50
+
+
 # ------------------------------------------------------------------------------- P7: fp32 values -------
 def test_fp32_values_path(tl, cfg0):
     va32 = cfg0["va"].astype(np.float32)
