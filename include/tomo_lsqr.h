@@ -97,7 +97,8 @@ tomo_status_t tomo_lsmr_solve(tomo_lsqr_t h, const double* d_b, double damp, dou
 tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
                                    int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream);
 
-/* a8: nrhs (1..8) independent LSQR recurrences sharing each pass over A / A^T (BASELINE configs[3]).
+/* a8: nrhs (1..8) independent LSQR recurrences sharing each pass over A / A^T (BASELINE configs[3]): one SpMM
+ * per product on row-major len x 8 blocks (fewer sides are padded with zero columns).
  * d_B fp64[m x nrhs] row-major, d_X fp64[n x nrhs] row-major, res[nrhs].  Every right-hand side stops
  * on its own tests; iterates of a stopped side are frozen. */
 tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
@@ -118,6 +119,8 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *                          the order-independent iterate that parity at fixed k is claimed for)
  *   "graph"       0 | 1    replay a CUDA graph (default 1) or launch kernel by kernel
  *   "profile"     0 | 1    1: kernel-by-kernel launches bracketed by CUDA events (see tomo_lsqr_get_info)
+ *   "multi_shared" 0 | 1   tomo_lsqr_solve_multi: 1 (default) the sides share every pass over A and A^T (SpMM on
+ *                          len x 8 blocks); 0 runs them one after the other (same results)
  *   "row_cost"    c >= 0   weight of a row, in elements, in the cost-balanced element split of the
  *                          persistent CTAs (default 96); changes the summation order only */
 tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value);

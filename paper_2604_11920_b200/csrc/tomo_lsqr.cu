@@ -17,6 +17,7 @@
 #include "build.cuh"
 #include "kernels.cuh"
 #include "stream.cuh"
+#include "multi.cuh"
 
 using namespace tomo;
 
@@ -63,6 +64,10 @@ struct tomo_lsqr_s {
   // work vectors and device state
   double *u = nullptr, *v = nullptr, *w = nullptr, *x = nullptr, *hbar = nullptr;  // w doubles as LSMR's h
   int solver = 0;  // 0 LSQR, 1 LSMR (set per solve)
+  // shared-pass multi-RHS state (multi.cuh): len x 8 blocks, eight Scalars, static row partitions
+  double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr; Scalars* msc = nullptr; Scalars* h_msc = nullptr;
+  int32_t *mpart_r = nullptr, *mpart_c = nullptr; double2* mpartials = nullptr; int MG = 0, multi_shared = 1;
+  cudaGraphExec_t mgexec = nullptr; int mgraph_k = 0, mgraph_mode = -1;
   Scalars* sc = nullptr; double2* part_spmv = nullptr; double2* part_vec = nullptr; int part_cap = 0;
   double *hist_r2 = nullptr, *hist_ar = nullptr; int32_t hist_cap = 0;
   double *bh = nullptr, *xh = nullptr;   // device staging for solve_host
@@ -204,6 +209,8 @@ void free_handle(tomo_lsqr_s* h) {
   for (int i = 0; i < 2; ++i) if (h->ev_poll[i]) cudaEventDestroy(h->ev_poll[i]);
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
   cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
+  cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->msc); cudaFree(h->mpart_r); cudaFree(h->mpart_c);
+  cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
   cudaFree(h->sE_r); cudaFree(h->sE_c); cudaFree(h->sR_r); cudaFree(h->sR_c); cudaFree(h->cta_rec);
   cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x); cudaFree(h->hbar);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
@@ -513,6 +520,106 @@ __global__ void k_col_scatter(const double* __restrict__ in, int nrhs, int r, in
 
 }  // namespace
 
+namespace {
+
+template <int OP>
+void launch_spmm(const tomo_lsqr_s* h, bool transpose, const double* X, double* Y, cudaStream_t st) {
+  const int64_t* ptr = transpose ? h->colptr : h->rowptr;
+  const int32_t* idx = transpose ? h->rowind : h->colind;
+  const int32_t* part = transpose ? h->mpart_c : h->mpart_r;
+  if (h->vt == TOMO_VAL_F64) {
+    const double* val = (const double*)(transpose ? h->cvals : h->vals);
+    if (h->accumulate) k_spmm8<1, double, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+    else k_spmm8<0, double, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+  } else {
+    const float* val = (const float*)(transpose ? h->cvals : h->vals);
+    if (h->accumulate) k_spmm8<1, float, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+    else k_spmm8<0, float, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+  }
+}
+
+template <int VOP>
+void launch_vec8(const tomo_lsqr_s* h, const double* in0, int nrhs, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st) {
+  const int g = (int)std::max<int64_t>(1, std::min<int64_t>((len * kR + kMThreads - 1) / kMThreads, (int64_t)h->MG));
+  if (h->accumulate) k_vec8<1, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials);
+  else k_vec8<0, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials);
+}
+
+void enqueue_multi_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
+  launch_spmm<OP_K1>(h, false, h->mV, h->mU, st);
+  launch_spmm<OP_K2>(h, true, h->mU, h->mV, st);
+  launch_vec8<VOP_K4>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st);
+}
+
+// Eight recurrences sharing every pass over A and A^T (multi.cuh).  nrhs < 8 is padded with zero columns.
+tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int32_t nrhs, const double* d_B, double damp, double atol, double btol,
+                                 int32_t max_iters, double* d_X, tomo_lsqr_result_t* res, cudaStream_t st) {
+  const int64_t m = h->m, n = h->n;
+  if (!h->mU) {
+    CK(cudaMalloc(&h->mU, sizeof(double) * m * kR)); CK(cudaMalloc(&h->mV, sizeof(double) * n * kR));
+    CK(cudaMalloc(&h->mW, sizeof(double) * n * kR)); CK(cudaMalloc(&h->mX, sizeof(double) * n * kR));
+    CK(cudaMalloc(&h->msc, sizeof(Scalars) * kR)); CK(cudaMallocHost(&h->h_msc, sizeof(Scalars) * kR));
+    h->MG = h->sms * 4;
+    CK(cudaMalloc(&h->mpart_r, sizeof(int32_t) * (h->MG + 1))); CK(cudaMalloc(&h->mpart_c, sizeof(int32_t) * (h->MG + 1)));
+    CK(cudaMalloc(&h->mpartials, sizeof(double2) * kR * h->MG));
+    const int tb = 128, gb = (h->MG + 1 + tb - 1) / tb;
+    k_partition<<<gb, tb, 0, st>>>(h->rowptr, m, h->MG, 16, 1, h->mpart_r);
+    k_partition_fix<<<1, 32, 0, st>>>(h->MG, h->mpart_r);
+    k_partition<<<gb, tb, 0, st>>>(h->colptr, n, h->MG, 16, 1, h->mpart_c);
+    k_partition_fix<<<1, 32, 0, st>>>(h->MG, h->mpart_c);
+    CK(cudaGetLastError());
+  }
+  const int k = h->check_every;
+  if (h->use_graph && !(h->mgexec && h->mgraph_k == k && h->mgraph_mode == h->accumulate)) {
+    if (h->mgexec) { cudaGraphExecDestroy(h->mgexec); h->mgexec = nullptr; }
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
+    for (int i = 0; i < k; ++i) enqueue_multi_iteration(h, h->cap_stream);
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&h->mgexec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { h->mgexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    h->mgraph_k = k; h->mgraph_mode = h->accumulate;
+  }
+  Scalars* hs = h->h_msc;
+  memset(hs, 0, sizeof(Scalars) * kR);
+  for (int r = 0; r < kR; ++r) { hs[r].damp = damp; hs[r].atol = atol; hs[r].btol = btol; hs[r].max_iters = max_iters; hs[r].cs2 = -1.0; }
+  CK(cudaMemcpyAsync(h->msc, hs, sizeof(Scalars) * kR, cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(h->mX, 0, sizeof(double) * n * kR, st));
+  CK(cudaMemsetAsync(h->mV, 0, sizeof(double) * n * kR, st));
+  CK(cudaMemsetAsync(h->mW, 0, sizeof(double) * n * kR, st));
+  launch_vec8<VOP_INIT_U>(h, d_B, nrhs, h->mU, nullptr, nullptr, m, st);
+  launch_spmm<OP_K2_INIT>(h, true, h->mU, h->mV, st);
+  launch_vec8<VOP_INIT_VW>(h, nullptr, kR, h->mV, h->mW, nullptr, n, st);
+  CK(cudaGetLastError());
+  h->kernels_enqueued += 3;
+  const int chunks = max_iters > 0 ? (max_iters + k - 1) / k : 0;
+  for (int c = 0; c < chunks; ++c) {
+    if (h->use_graph) CK(cudaGraphLaunch(h->mgexec, st));
+    else { for (int i = 0; i < k; ++i) enqueue_multi_iteration(h, st); CK(cudaGetLastError()); }
+    h->kernels_enqueued += 3.0 * k;
+    // poll: the eight {itn, istop, stop} words; stop when every side has stopped
+    CK(cudaMemcpy2DAsync(h->h_msc, sizeof(Scalars), h->msc, sizeof(Scalars), sizeof(Scalars), kR, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    bool all = true;
+    for (int r = 0; r < kR; ++r) all = all && (h->h_msc[r].stop != 0);
+    if (all) break;
+  }
+  CK(cudaMemcpyAsync(h->h_msc, h->msc, sizeof(Scalars) * kR, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpy2DAsync(d_X, sizeof(double) * nrhs, h->mX, sizeof(double) * kR, sizeof(double) * nrhs, n, cudaMemcpyDeviceToDevice, st));
+  CK(cudaStreamSynchronize(st));
+  if (res)
+    for (int r = 0; r < nrhs; ++r) {
+      const Scalars& q = h->h_msc[r];
+      res[r].itn = q.itn; res[r].istop = q.istop; res[r].r1norm = q.r1norm; res[r].r2norm = q.r2norm;
+      res[r].arnorm = q.arnorm; res[r].anorm = q.anorm; res[r].acond = q.acond; res[r].xnorm = q.xnorm;
+    }
+  return TOMO_OK;
+}
+
+}  // namespace
+
 extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
                                                double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
                                                void* cuda_stream) {
@@ -521,6 +628,7 @@ extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, cons
   if (nrhs < 1 || nrhs > 8 || !d_B || !d_X) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_B) || !is_device_ptr(d_X)) return TOMO_ERR_NOT_DEVICE_PTR;
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->multi_shared) return solve_multi_shared(h, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, st);
   if (!h->bh) CK(cudaMalloc(&h->bh, sizeof(double) * h->m));
   if (!h->xh) CK(cudaMalloc(&h->xh, sizeof(double) * h->n));
   for (int r = 0; r < nrhs; ++r) {
@@ -565,6 +673,7 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; if (h->accumulate != (int)value) h->part_dirty = true; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
+  else if (k == "multi_shared") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->multi_shared = (int)value; }
   else if (k == "row_cost") { if (value < 0 || value > 4096) return TOMO_ERR_INVALID_ARG; if (h->row_cost != (int)value) h->part_dirty = true; h->row_cost = (int)value; }
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
