@@ -2,7 +2,7 @@
 // LSQR recurrences that SHARE every pass over A and A^T.  Vectors are row-major blocks (len x 8): one
 // element of the matrix is read once and multiplied with a 64-byte row of the gathered block, so the
 // HBM stream of `idx`/`val` is paid once per iteration for all eight systems; the gather (64 B per
-// nonzero from L1/L2) and, in dd mode, the fp64 pipe become the limits.
+// nonzero through L1/L2) and, in dd mode, the fp64 pipe become the limits.
 //
 // Each right-hand side has its own device-resident Scalars (sc[0..8)), its own stopping tests and stop
 // flag; a stopped side is frozen: its columns are no longer written.  Fewer than eight sides are padded
@@ -17,29 +17,6 @@ namespace tomo {
 constexpr int kR = 8;             // right-hand sides per pass
 constexpr int kMThreads = 256;    // block size of the multi kernels
 constexpr int kMWarps = kMThreads / 32;
-
-// Per-column sums of 8 accumulators held by every lane -> lane k (< 8) ends up with the warp total of
-// column k.  Butterfly over the 32 lanes, fixed order.
-template <int MODE>
-__device__ __forceinline__ Acc<MODE> warp_columns(Acc<MODE> (&a)[kR], int lane) {
-#pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) {
-#pragma unroll
-    for (int k = 0; k < kR; ++k) {
-      Acc<MODE> o;
-      double2 p = a[k].pack();
-      p.x = __shfl_xor_sync(0xffffffffu, p.x, off);
-      p.y = __shfl_xor_sync(0xffffffffu, p.y, off);
-      o.unpack(p);
-      // both partners must add in the same order to stay bitwise identical: lower lane's value first
-      if (lane & off) { o.merge(a[k]); a[k] = o; } else { a[k].merge(o); }
-    }
-  }
-  Acc<MODE> r = a[0];
-#pragma unroll
-  for (int k = 1; k < kR; ++k) if ((lane & 7) == k) r = a[k];
-  return r;
-}
 
 // block-level: lanes 0..7 of every warp hold a per-column partial -> thread k (< 8) returns the block sum
 template <int MODE>
