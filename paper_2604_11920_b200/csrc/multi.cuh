@@ -97,16 +97,16 @@ __global__ void __launch_bounds__(kMThreads) k_spmm8(const int64_t* __restrict__
     Acc<MODE> a0, a1;
     a0.zero(); a1.zero();
     int64_t q = s + es;
-    for (; q + 24 < e; q += 32) {  // four steps in flight
-      int32_t cc[4];
-      double vv[4];
-      double2 xx[4];
+    for (; q + 56 < e; q += 64) {  // eight steps in flight
+      int32_t cc[8];
+      double vv[8];
+      double2 xx[8];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) { cc[u] = idx[q + 8 * u]; vv[u] = (double)val[q + 8 * u]; }
+      for (int u = 0; u < 8; ++u) { cc[u] = idx[q + 8 * u]; vv[u] = (double)val[q + 8 * u]; }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) xx[u] = __ldg(X2 + (size_t)cc[u] * (kR / 2) + j);
+      for (int u = 0; u < 8; ++u) xx[u] = __ldg(X2 + (size_t)cc[u] * (kR / 2) + j);
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < 8; ++u) {
         if (SCALE_X) { xx[u].x = xx[u].x * sx0; xx[u].y = xx[u].y * sx1; }
         a0.mac(vv[u], xx[u].x);
         a1.mac(vv[u], xx[u].y);
