@@ -559,7 +559,7 @@ tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int32_t nrhs, const double* d_B
     CK(cudaMalloc(&h->mU, sizeof(double) * m * kR)); CK(cudaMalloc(&h->mV, sizeof(double) * n * kR));
     CK(cudaMalloc(&h->mW, sizeof(double) * n * kR)); CK(cudaMalloc(&h->mX, sizeof(double) * n * kR));
     CK(cudaMalloc(&h->msc, sizeof(Scalars) * kR)); CK(cudaMallocHost(&h->h_msc, sizeof(Scalars) * kR));
-    h->MG = h->sms * 4;
+    h->MG = h->sms * 8;
     CK(cudaMalloc(&h->mpart_r, sizeof(int32_t) * (h->MG + 1))); CK(cudaMalloc(&h->mpart_c, sizeof(int32_t) * (h->MG + 1)));
     CK(cudaMalloc(&h->mpartials, sizeof(double2) * kR * h->MG));
     const int tb = 128, gb = (h->MG + 1 + tb - 1) / tb;
