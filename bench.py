@@ -55,19 +55,26 @@ def measured_peak_gbs() -> tuple[float, str]:
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic_bytes(config: int):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+def ncu_traffic_bytes(config: int, nrhs: int = 1):
+    """(dram bytes per launch of the dominant kernel, where the number comes from) read from the committed ncu
+    --set full summary profiles/dram_traffic.csv: a figure captured ONCE per kernel generation under ncu, not in
+    this run (a number taken under a profiler is never a bench value).  (None, reason) if there is no entry."""
     p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    key = "k_wstream_mean_bytes_per_launch" if nrhs == 1 else "k_spmm8_mean_bytes_per_launch"
     if not os.path.exists(p):
-        return None
+        return None, "profiles/dram_traffic.csv missing"
     try:
+        src = ""
         for line in open(p):
+            if line.startswith("#"):
+                src = line.lstrip("# ").strip()
+                continue
             f = [t.strip() for t in line.split(",")]
-            if len(f) >= 3 and f[0] == f"cfg{config}" and f[1] == "k_stream_mean_bytes_per_launch":
-                return float(f[2])
-    except Exception:
-        return None
-    return None
+            if len(f) >= 3 and f[0] == f"cfg{config}" and f[1] == key:
+                return float(f[2]), f"profiles/dram_traffic.csv ({src})"
+    except Exception as e:  # noqa: BLE001
+        return None, f"unreadable: {e}"
+    return None, f"no {key} entry for cfg{config} in profiles/dram_traffic.csv"
 
 
 class ClockSampler:
@@ -177,8 +184,129 @@ def run_reference(args) -> dict:
     }
 
 
+def block_bytes(m: int, n: int, nnz: int, nrhs: int, vbytes: int = 8) -> dict:
+    """Algorithmic bytes of one BLOCK iteration of the shared-pass multi-RHS solve (the matrix
+    streams once for all sides, the vector traffic nrhs times): 24 nnz + 8 (32 m + 72 n) at nrhs = 8, fp64."""
+    k1 = (vbytes + 4) * nnz + 8 * (m + 1) + nrhs * 8 * (2 * m + n)
+    k2 = (vbytes + 4) * nnz + 8 * (n + 1) + nrhs * 8 * (2 * n + m)
+    return dict(k1=k1, k2=k2, k4=nrhs * 40 * n, iteration=k1 + k2 + nrhs * 40 * n)
+
+
+def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, both_modes=True):
+    """Times args.config-style steps on system `s` (already chosen); returns the raw numbers of one workload."""
+    m, n, nnz = s.dims.m, s.dims.n, s.dims.nnz
+    damp, atol, btol, max_iters = s.damp, s.solve["atol"], s.solve["btol"], s.solve["max_iters"]
+    nrhs = s.dims.nrhs
+    b_host = torch.from_numpy(s.rhs(0)).pin_memory()
+    x_host = torch.empty(n, dtype=torch.float64).pin_memory()
+    rp_d, ci_d, va_d = s.csr_cuda()  # generated and uploaded block by block (config 2: 45 GB)
+    vbytes = 8
+    if args.vals == "f32":  # optional fp32 storage of the values (arithmetic stays fp64)
+        va_d, vbytes = va_d.to(torch.float32), 4
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    S = tl.TomoLsqr(m, n, rp_d, ci_d, va_d)
+    torch.cuda.synchronize()
+    create_wall_ms = 1e3 * (time.perf_counter() - t0)
+    S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=args.compress)
+    if args.row_cost is not None:
+        S.set(row_cost=args.row_cost)
+    b = b_host.cuda()
+    x = torch.empty(n, dtype=torch.float64, device="cuda")
+    lsmr = args.solver == "lsmr"
+
+    class _Its:  # a step's iteration count (all right-hand sides)
+        def __init__(self, itn):
+            self.itn = itn
+
+    if nrhs > 1:  # configs[3]: 8 recurrences sharing every pass over A and A^T (DESIGN.md a8)
+        B_host = torch.from_numpy(s.rhs_block()).pin_memory()
+        X_host = torch.empty((n, nrhs), dtype=torch.float64).pin_memory()
+        B = B_host.cuda()
+        X = torch.empty((n, nrhs), dtype=torch.float64, device="cuda")
+        multi = tl.tomo_lsmr_solve_multi if lsmr else tl.tomo_lsqr_solve_multi
+
+    def step_device():
+        if nrhs > 1:
+            return _Its(sum(r.itn for r in multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
+        return (tl.tomo_lsmr_solve if lsmr else tl.tomo_lsqr_solve)(S.h, b, damp, atol, btol, max_iters, x)
+
+    def step_host():
+        if nrhs > 1:  # the block solve has no host-buffer entry: pinned copies around the device call, inside the timed region
+            B.copy_(B_host, non_blocking=True)
+            r = _Its(sum(r.itn for r in multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
+            X_host.copy_(X)
+            return r
+        return (tl.tomo_lsmr_solve_host if lsmr else tl.tomo_lsqr_solve_host)(S.h, b_host, damp, atol, btol, max_iters, x_host)
+
+    def timed(step):
+        for _ in range(warmup):
+            step()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0 = S.info("kernels_enqueued")
+        e0.record()
+        its = 0
+        for _ in range(steps):
+            its += step().itn
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        launches = S.info("kernels_enqueued") - k0
+        if dist is not None:
+            ms, its, launches = aggregate_over_ranks(dist, ms, its, launches, device="cuda")
+        return ms, its, launches
+
+    out = {"m": m, "n": n, "nnz": nnz, "nrhs": nrhs, "vbytes": vbytes, "create_wall_ms": create_wall_ms,
+           "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms")}
+    with ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) as clk:
+        out["ms"], out["its"], out["launches"] = timed(step_device)
+    out["clocks"] = clk.summary()
+    if e2e:
+        out["ms_e2e"], out["its_e2e"], _ = timed(step_host)
+    # per-kernel durations, live: the same solve launched kernel by kernel with CUDA events around each launch on
+    # the launching stream (library option "profile"); for the block solve these are the k_spmm8 / k_vec8 launches
+    S.set(profile=1)
+    for _ in range(2):
+        step_device()
+    nl = max(S.info("k_launches"), 1.0)
+    out["k1_us"], out["k2_us"], out["k4_us"] = (1e3 * S.info(k) / nl for k in ("k1_ms", "k2_ms", "k4_ms"))
+    S.set(profile=0)
+    if both_modes:  # the other accumulation mode, for context
+        S.set(accumulate=1 - args.accumulate)
+        ms_o, its_o, _ = timed(step_device)
+        out["other"] = {"accumulate": 1 - args.accumulate, "value": its_o / (ms_o * 1e-3), "ms_per_step": ms_o / steps}
+        S.set(accumulate=args.accumulate)
+    if args.compress:
+        out["index_bytes"] = (S.info("compress_bytes_rows"), S.info("compress_bytes_cols"))
+    S.close()
+    return out
+
+
+def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
+    """The roofline object of one measured workload: algorithmic bytes of the two sparse launches of an iteration
+     over their live CUDA-event time."""
+    m, n, nnz, nrhs, vb = r["m"], r["n"], r["nnz"], r["nrhs"], r["vbytes"]
+    ab = algorithmic_bytes(m, n, nnz, vb) if nrhs == 1 else block_bytes(m, n, nnz, nrhs, vb)
+    note = "general CSR byte count: (values + int32 index) per nonzero + pointers + vectors"
+    if compress and "index_bytes" in r:  # NEXT-2: its own byte count, never mixed into the CSR roofline
+        ab = dict(ab)
+        ab["k1"] += int(r["index_bytes"][0]) - 4 * nnz
+        ab["k2"] += int(r["index_bytes"][1]) - 4 * nnz
+        note = "run-compressed index (option compress=1): values + measured compressed index bytes + pointers + vectors"
+    spmv_bytes = ab["k1"] + ab["k2"]
+    achieved = spmv_bytes / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e9
+    kern = ("k_wstream (K1: A v - alpha u + norm over CSR; K2: A^T u - beta v + norm over CSC), mean of the two launches of an iteration"
+            if nrhs == 1 else
+            "k_spmm8 (the same two products on len x 8 blocks, 8 right-hand sides per pass), mean of the two launches of a block iteration")
+    return {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "algorithmic_bytes_per_launch": spmv_bytes / 2, "byte_count": note, "peak_source": peak_src,
+            "frac_of_8TBs": achieved / 8000.0, "bytes_per_launch_pair": spmv_bytes,
+            "k1_us": r["k1_us"], "k2_us": r["k2_us"], "k4_us": r["k4_us"],
+            "k1_gbs": ab["k1"] / (r["k1_us"] * 1e-6) / 1e9, "k2_gbs": ab["k2"] / (r["k2_us"] * 1e-6) / 1e9}
+
+
 def run_ours(args) -> dict | None:
-    import numpy as np
     import torch
     import paper_2604_11920_b200 as tl
     tl.load()  # raises if libtomolsqr.so is missing: there is no fallback
@@ -201,143 +329,106 @@ def run_ours(args) -> dict | None:
 
     import tomogen
     s = tomogen.System(args.config)
-    m, n, nnz = s.dims.m, s.dims.n, s.dims.nnz
-    damp, atol, btol, max_iters = s.damp, s.solve["atol"], s.solve["btol"], s.solve["max_iters"]
-    b_host = torch.from_numpy(s.rhs(0)).pin_memory()
-    x_host = torch.empty(n, dtype=torch.float64).pin_memory()
-    rp_d, ci_d, va_d = s.csr_cuda()  # generated and uploaded block by block (config 2: 45 GB)
-    vbytes = 8
-    if args.vals == "f32":  # optional fp32 storage of the values (arithmetic stays fp64)
-        va_d, vbytes = va_d.to(torch.float32), 4
-    S = tl.TomoLsqr(m, n, rp_d, ci_d, va_d)
-    S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0)
-    if args.row_cost is not None:
-        S.set(row_cost=args.row_cost)
-    b = b_host.cuda()
-    x = torch.empty(n, dtype=torch.float64, device="cuda")
+    r = measure(tl, torch, s, args, barrier, dist, world, args.steps, args.warmup, e2e=True, both_modes=args.both_modes)
+    m, n, nnz, nrhs, vbytes = r["m"], r["n"], r["nnz"], r["nrhs"], r["vbytes"]
+    ms, its = r["ms"], r["its"]
 
-    nrhs = s.dims.nrhs
-
-    class _Its:  # a step's iteration count (all right-hand sides)
-        def __init__(self, itn):
-            self.itn = itn
-
-    if nrhs > 1:  # configs[3]: the 8 right-hand sides (DESIGN.md a8: eight recurrences sharing every pass over A and A^T)
-        B_host = torch.from_numpy(s.rhs_block()).pin_memory()
-        X_host = torch.empty((n, nrhs), dtype=torch.float64).pin_memory()
-        B = B_host.cuda()
-        X = torch.empty((n, nrhs), dtype=torch.float64, device="cuda")
-
-    def step_device():
-        if nrhs > 1:
-            return _Its(sum(r.itn for r in tl.tomo_lsqr_solve_multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
-        if args.solver == "lsmr":
-            return tl.tomo_lsmr_solve(S.h, b, damp, atol, btol, max_iters, x)
-        return tl.tomo_lsqr_solve(S.h, b, damp, atol, btol, max_iters, x)
-
-    def step_host():
-        if args.solver == "lsmr":  # no host-buffer entry for LSMR: copies around the device call
-            b.copy_(b_host, non_blocking=True)
-            r = tl.tomo_lsmr_solve(S.h, b, damp, atol, btol, max_iters, x)
-            x_host.copy_(x)
-            return r
-        if nrhs > 1:  # no host-buffer entry for the block solve: copies around the device call
-            B.copy_(B_host, non_blocking=True)
-            r = _Its(sum(r.itn for r in tl.tomo_lsqr_solve_multi(S.h, nrhs, B, damp, atol, btol, max_iters, X)))
-            X_host.copy_(X)
-            return r
-        return tl.tomo_lsqr_solve_host(S.h, b_host, damp, atol, btol, max_iters, x_host)
-
-    def timed(step):
-        for _ in range(args.warmup):
-            step()
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        k0 = S.info("kernels_enqueued")
-        e0.record()
-        its = 0
-        for _ in range(args.steps):
-            its += step().itn
-        e1.record()
-        barrier()
-        ms = e0.elapsed_time(e1)
-        launches = S.info("kernels_enqueued") - k0
-        if dist is not None:
-            ms, its, launches = aggregate_over_ranks(dist, ms, its, launches, device="cuda")
-        return ms, its, launches
-
-    with ClockSampler(local) as clk:
-        ms, its, launches = timed(step_device)
-    clocks = clk.summary()
-    ms_e2e, its_e2e, _ = timed(step_host)
-
-    # per-kernel durations, live: the same solve launched kernel by kernel with CUDA events around each
-    # launch on the launching stream (library option "profile")
-    S.set(profile=1)
-    for _ in range(2):
-        if nrhs > 1:  # the block solve has no per-kernel read-out: time the single-side kernels on column 0
-            tl.tomo_lsqr_solve(S.h, B[:, 0].contiguous(), damp, atol, btol, max_iters, x)
-        else:
-            step_device()
-    nl = S.info("k_launches")
-    k1_us, k2_us, k4_us = (1e3 * S.info(k) / nl for k in ("k1_ms", "k2_ms", "k4_ms"))
-    S.set(profile=0)
-    # fast-mode (plain fp64 FMA) numbers for context
-    other = {}
-    if args.both_modes:
-        S.set(accumulate=1 - args.accumulate)
-        ms_o, its_o, _ = timed(step_device)
-        other = {"accumulate": 1 - args.accumulate, "value": its_o / (ms_o * 1e-3), "ms_per_step": ms_o / args.steps}
-        S.set(accumulate=args.accumulate)
+    also = {}
+    if world == 1 and args.config == 1 and not args.no_also and torch.cuda.mem_get_info()[1] >= 150e9:
+        # BASELINE.json north_star names configs[1] AND configs[2] for the >= 60 % target: the large system, 2 steps
+        torch.cuda.empty_cache()
+        s2 = tomogen.System(2)
+        r2 = measure(tl, torch, s2, args, barrier, None, 1, 2, 3, e2e=False, both_modes=True)
+        peak2, src2 = measured_peak_gbs()
+        rf2 = roofline_of(r2, peak2, src2, args.compress)
+        also["configs[2]"] = {"workload": workload_name(s2), "value": r2["its"] / (r2["ms"] * 1e-3), "unit": UNIT,
+                              "accumulate": args.accumulate, "other_mode": r2.get("other"), "ms_per_step": r2["ms"] / 2, "steps": 2,
+                              "warmup": 3, "k1_us": r2["k1_us"], "k2_us": r2["k2_us"], "k4_us": r2["k4_us"],
+                              "achieved_gbs": rf2["achieved"], "frac": rf2["frac"], "frac_of_8TBs": rf2["frac_of_8TBs"],
+                              "create_ms": r2["create_ms"], "transpose_ms": r2["transpose_ms"], "clocks": r2["clocks"]}
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return None
 
-    ab = algorithmic_bytes(m, n, nnz, vbytes)
     peak, peak_src = measured_peak_gbs()
-    spmv_bytes = ab["k1"] + ab["k2"]
-    achieved = spmv_bytes / ((k1_us + k2_us) * 1e-6) / 1e9
-    if nrhs > 1:  # shared pass: the matrix stream once per block iteration, the vector traffic nrhs times
-        block_bytes = 2 * (vbytes + 4) * nnz + 8 * (m + n + 2) + nrhs * 8 * (3 * m + 3 * n + 5 * n)
-        achieved = block_bytes * (its / nrhs / world) / (ms * 1e-3) / 1e9
-    traffic = ncu_traffic_bytes(args.config)
+    rf = roofline_of(r, peak, peak_src, args.compress)
+    rf["traffic"], rf["traffic_source"] = ncu_traffic_bytes(args.config, nrhs)
+    ab = algorithmic_bytes(m, n, nnz, vbytes) if nrhs == 1 else block_bytes(m, n, nnz, nrhs, vbytes)
+    # bytes moved per second by the whole step: single side per iteration, block solve per BLOCK iteration (its / nrhs)
+    eff = ab["iteration"] * (its / nrhs) / world / (ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": workload_name(s), "iterations_per_step": its // max(1, args.steps * world),
                    "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
-                   "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs, "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic", "parallelism": "replicas" if world > 1 else "single GPU",
+                   "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
+                   "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
+                   "index": "run-compressed (compress=1)" if args.compress else "int32 per nonzero",
+                   "parallelism": "replicas" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {ab['iteration'] / 1e9:.2f} GB streamed per iteration vs 126 MB L2, no flush needed"},
-        "effective_gbs": ab["iteration"] * its / world / (ms * 1e-3) / 1e9,
-        "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms"),
-        "e2e": {"value": its_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * m * nrhs, "d2h_bytes_per_step": 8 * n * nrhs,
-                "ms_per_step": ms_e2e / args.steps},
-        "gpu_launches": int(launches),
-        "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "k_stream (K1: A v - alpha u + norm over CSR; K2: A^T u - beta v + norm over CSC), mean of the two launches of an iteration",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
-                     "algorithmic_bytes_per_launch": spmv_bytes / 2,
-                     "peak_source": peak_src, "frac_of_8TBs": achieved / 8000.0,
-                     "bytes_per_launch_pair": spmv_bytes, "k1_us": k1_us, "k2_us": k2_us, "k4_us": k4_us,
-                     "k1_gbs": ab["k1"] / (k1_us * 1e-6) / 1e9, "k2_gbs": ab["k2"] / (k2_us * 1e-6) / 1e9},
+        "effective_gbs": eff,
+        "create_ms": r["create_ms"], "transpose_ms": r["transpose_ms"], "create_wall_ms": r["create_wall_ms"],
+        "create_note": "create_ms / transpose_ms: CUDA events inside tomo_lsqr_create (kernels + its cudaMalloc calls); create_wall_ms: host clock around the call",
+        "e2e": {"value": r["its_e2e"] / (r["ms_e2e"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * m * nrhs,
+                "d2h_bytes_per_step": 8 * n * nrhs, "ms_per_step": r["ms_e2e"] / args.steps},
+        "gpu_launches": int(r["launches"]),
+        "clocks": r["clocks"],
+        "roofline": rf,
     }
-    if other:
-        out["other_mode"] = other
+    if "other" in r:
+        out["other_mode"] = r["other"]
+    if also:
+        out["also"] = also
     if world == 1 and not args.no_cpu:
         import oracle
         iters = ref_iters_for(args)
         rp, ci, va = s.csr()
         t0 = time.perf_counter()
-        r = oracle.lsqr(m, n, rp, ci, va, s.rhs(0), damp=damp, atol=0.0, btol=0.0, max_iters=iters, mode=oracle.PLAIN)
+        ro = oracle.lsqr(m, n, rp, ci, va, s.rhs(0), damp=s.damp, atol=0.0, btol=0.0, max_iters=iters, mode=oracle.PLAIN)
         dt = time.perf_counter() - t0
-        out["cpu_baseline"] = {"value": r.itn / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+        out["cpu_baseline"] = {"value": ro.itn / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": f"{iters} iterations (plus the init pass) of the full configs[{args.config}] system, plain fp64 mode"}
     if dist is not None:
         dist.destroy_process_group()
     return out
+
+
+def relaunch_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun around it: start the N ranks here (one process per
+    GPU, NCCL for the timing reduction) and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")  # communicator lines stay visible (rank count evidence)
+    return subprocess.call(cmd, env=env)
+
+
+def run_stub(args) -> dict | None:
+    """TEST-ONLY (tests/test_bench_ranks.py, `--stub-step`): the rank plumbing of the N > 1 path — environment,
+    process group (gloo, CPU), barrier, max / sum aggregation, rank 0 prints — with a step that does NO work and
+    touches neither the GPU nor the library.  Its line says "stub": true and carries no value."""
+    import torch
+    import torch.distributed as dist
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    ms, its, launches = 10.0 * (rank + 1), 7 * args.steps, 21.0 * args.steps
+    if world > 1:
+        ms, its, launches = aggregate_over_ranks(dist, ms, its, launches, device="cpu")
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+    return {"stub": True, "metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "scaling": "weak", "stub_iterations": its, "stub_launches": launches}
 
 
 def main():
@@ -350,11 +441,14 @@ def main():
     ap.add_argument("--accumulate", type=int, default=1, choices=[0, 1])
     ap.add_argument("--check-every", dest="check_every", type=int, default=10)
     ap.add_argument("--ref-iters", dest="ref_iters", type=int, default=20)
-    ap.add_argument("--both-modes", dest="both_modes", action="store_true", default=True)
+    ap.add_argument("--one-mode", dest="both_modes", action="store_false", default=True, help="skip the other accumulation mode")
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
+    ap.add_argument("--no-also", dest="no_also", action="store_true", help="skip the configs[2] lines attached to a configs[1] run")
     ap.add_argument("--solver", default="lsqr", choices=["lsqr", "lsmr"], help="lsqr (BASELINE metric) or lsmr (the paper's solver)")
     ap.add_argument("--vals", default="f64", choices=["f64", "f32"], help="storage type of the matrix values")
+    ap.add_argument("--compress", type=int, default=0, choices=[0, 1], help="1: run-compressed index (NEXT-2), reported with its own byte count")
     ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
+    ap.add_argument("--stub-step", dest="stub", action="store_true", help="TEST-ONLY: rank plumbing with a step that does no work (no GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -362,7 +456,9 @@ def main():
             return
         print(json.dumps(run_reference(args)), flush=True)
         return
-    out = run_ours(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(relaunch_under_torchrun(args))
+    out = run_stub(args) if args.stub else run_ours(args)
     if out is not None:
         print(json.dumps(out), flush=True)
 

@@ -24,11 +24,14 @@
  *   Ownership: the three CSR arrays are BORROWED: the caller keeps them alive and unmodified until
  *          tomo_lsqr_destroy.  The handle owns the CSC copy, the work vectors, the scalars, the graphs.
  *          Output arrays (d_x, d_out, d_X) are caller-allocated and fully overwritten.
- *   Errors: status codes only; no exceptions, no abort.  On error, *out is NULL / outputs are unspecified.
+ *   Errors: status codes only; no exceptions, no abort.  On error *out is NULL; argument errors (INVALID_ARG,
+ *          NOT_DEVICE_PTR, RANGE, BAD_CSR, UNSUPPORTED_ARCH) are detected before any work is enqueued, so the
+ *          output arrays are untouched; after TOMO_ERR_CUDA / TOMO_ERR_OOM their contents are unspecified.
  *   Streams: `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
  *          enqueued on it; solve* return after their last host poll, i.e. results are valid on return.
  *   Threads: one handle runs one call at a time; different handles are independent.
- *   Device: compute capability 10.x only (TOMO_ERR_UNSUPPORTED_ARCH otherwise; no fallback).
+ *   Device: compute capability 10.x only (TOMO_ERR_UNSUPPORTED_ARCH otherwise; no fallback).  A handle belongs
+ *          to the device that was current at create; calling it with another current device -> INVALID_ARG.
  */
 #ifndef TOMO_LSQR_H_
 #define TOMO_LSQR_H_
@@ -68,7 +71,7 @@ typedef struct {
   double xnorm;   /* ||x|| estimate */
 } tomo_lsqr_result_t;
 
-/* a0: validate the CSR arrays on the device, build the stable CSC transpose
+/* a0 (DESIGN.md §6.3 "create"): validate the CSR arrays on the device, build the stable CSC transpose
  * (rows ascending inside each column) and the cost-balanced element split points of the persistent CTAs.  One-off per matrix.
  * vt selects the storage type of d_vals (arithmetic is fp64 either way). */
 tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr,
@@ -92,9 +95,12 @@ tomo_status_t tomo_lsmr_solve(tomo_lsqr_t h, const double* d_b, double damp, dou
                               int32_t max_iters, double* d_x, tomo_lsqr_result_t* res, double* h_normr_hist,
                               double* h_normar_hist, void* cuda_stream);
 
-/* The same solve with HOST buffers: h_b fp64[m] is copied to the device, h_x fp64[n] is copied back
- * (the end-to-end entry bench.py times; the matrix stays resident in the handle). */
+/* The same solves with HOST buffers: h_b fp64[m] is copied to the device, h_x fp64[n] is copied back
+ * (the end-to-end entries bench.py times; the matrix stays resident in the handle).  tomo_lsmr_solve_host is
+ * the LSMR counterpart (the paper's solver). */
 tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
+                                   int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream);
+tomo_status_t tomo_lsmr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
                                    int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream);
 
 /* a8: nrhs (1..8) independent LSQR recurrences sharing each pass over A / A^T (BASELINE configs[3]): one SpMM
@@ -102,6 +108,10 @@ tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp
  * d_B fp64[m x nrhs] row-major, d_X fp64[n x nrhs] row-major, res[nrhs].  Every right-hand side stops
  * on its own tests; iterates of a stopped side are frozen. */
 tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
+                                    double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
+                                    void* cuda_stream);
+/* The same block solve by LSMR: per-side LSMR scalars, the three-vector update on len x 8 blocks. */
+tomo_status_t tomo_lsmr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
                                     double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
                                     void* cuda_stream);
 
@@ -121,12 +131,22 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *   "profile"     0 | 1    1: kernel-by-kernel launches bracketed by CUDA events (see tomo_lsqr_get_info)
  *   "multi_shared" 0 | 1   tomo_lsqr_solve_multi: 1 (default) the sides share every pass over A and A^T (SpMM on
  *                          len x 8 blocks); 0 runs them one after the other (same results)
+ *   "compress"    0 | 1    NEXT-2, the structure-exploiting operator: 1 builds (once, on the NULL stream)
+ *                          run-compressed copies of the column indices of the CSR and of the row indices of the CSC
+ *                          copy (one bit per element + one int32 per run of consecutive indices; the depth-fastest
+ *                          ordering of PAPER.md Eq. 7 P:79 makes every lateral node of a ray a run of consecutive
+ *                          columns, Eq. 5) and streams those instead of the int32 arrays.  Same elements,
+ *                          same order: results are bitwise those of "compress" = 0.  Default 0.
+ *   "pdl"         0 | 1    chain the kernels of an iteration with programmatic dependent launch (default 1): the
+ *                          prologue of a kernel (barrier set-up, split points, first bulk copies) overlaps the
+ *                          tail of the previous one; never changes results
  *   "row_cost"    c >= 0   weight of a row, in elements, in the cost-balanced element split of the
  *                          persistent CTAs (default 96); changes the summation order only */
 tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value);
 
 /* Read-outs (host double): "create_ms", "transpose_ms", "csc_bytes", "scratch_bytes", "blocks_rows",
- * "blocks_cols", and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
+ * "blocks_cols", "compress_bytes_rows" / "compress_bytes_cols" (bytes of the run-compressed index of each direction,
+ * 0 before "compress" was set), and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
  * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each);
  * "kernels_enqueued": cumulative number of kernel launches this handle has issued in solves (nodes of
  * replayed graphs included); "cta_busy_min" / "cta_busy_mean" / "cta_busy_max": busy cycles of the persistent

@@ -22,7 +22,8 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
-    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsqr_solve_multi", "tomo_lsqr_spmv",
+    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
+    "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
 )
 
@@ -56,7 +57,9 @@ def load() -> ctypes.CDLL:
     lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
     lib.tomo_lsmr_solve.argtypes = lib.tomo_lsqr_solve.argtypes
     lib.tomo_lsqr_solve_host.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
+    lib.tomo_lsmr_solve_host.argtypes = lib.tomo_lsqr_solve_host.argtypes
     lib.tomo_lsqr_solve_multi.argtypes = [vp, i32, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
+    lib.tomo_lsmr_solve_multi.argtypes = lib.tomo_lsqr_solve_multi.argtypes
     lib.tomo_lsqr_spmv.argtypes = [vp, ci, vp, vp, vp]
     lib.tomo_lsqr_get_csc.argtypes = [vp, vp, vp, vp, vp]
     lib.tomo_lsqr_set_option.argtypes = [vp, ctypes.c_char_p, i64]
@@ -133,11 +136,27 @@ def tomo_lsqr_solve_host(h, h_b, damp, atol, btol, max_iters, h_x, stream=None) 
     return res
 
 
+def tomo_lsmr_solve_host(h, h_b, damp, atol, btol, max_iters, h_x, stream=None) -> tomo_lsqr_result_t:
+    res = tomo_lsqr_result_t()
+    st = load().tomo_lsmr_solve_host(h, _ptr(h_b), damp, atol, btol, max_iters, _ptr(h_x), ctypes.byref(res), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsmr_solve_host")
+    return res
+
+
 def tomo_lsqr_solve_multi(h, nrhs, d_B, damp, atol, btol, max_iters, d_X, stream=None):
     res = (tomo_lsqr_result_t * nrhs)()
     st = load().tomo_lsqr_solve_multi(h, nrhs, _ptr(d_B), damp, atol, btol, max_iters, _ptr(d_X), res, _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_solve_multi")
+    return list(res)
+
+
+def tomo_lsmr_solve_multi(h, nrhs, d_B, damp, atol, btol, max_iters, d_X, stream=None):
+    res = (tomo_lsqr_result_t * nrhs)()
+    st = load().tomo_lsmr_solve_multi(h, nrhs, _ptr(d_B), damp, atol, btol, max_iters, _ptr(d_X), res, _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsmr_solve_multi")
     return list(res)
 
 
@@ -230,11 +249,12 @@ class TomoLsqr:
             return x, res, r2[: res.itn], ar[: res.itn]
         return x, res
 
-    def solve_multi(self, B, damp=0.0, atol=0.0, btol=0.0, max_iters=50):
+    def solve_multi(self, B, damp=0.0, atol=0.0, btol=0.0, max_iters=50, solver="lsqr"):
         import torch
         nrhs = B.shape[1]
         X = torch.empty((self.n, nrhs), dtype=torch.float64, device=B.device)
-        res = tomo_lsqr_solve_multi(self.h, nrhs, B.contiguous(), damp, atol, btol, max_iters, X)
+        fn = {"lsqr": tomo_lsqr_solve_multi, "lsmr": tomo_lsmr_solve_multi}[solver]
+        res = fn(self.h, nrhs, B.contiguous(), damp, atol, btol, max_iters, X)
         return X, [Result.of(r) for r in res]
 
     def close(self):

@@ -21,6 +21,13 @@ struct dd_t {
   double hi, lo;
 };
 
+// Programmatic dependent launch (the kernels of an iteration are chained with
+// cudaLaunchAttributeProgrammaticStreamSerialization): everything above grid_dependency_wait() may run while
+// the previous kernel drains; nothing that kernel writes is read before it.  launch_dependents() lets the next
+// kernel's CTAs start their prologue.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ void two_sum(double a, double b, double& s, double& t) {
   s = a + b;
   double bb = s - a;

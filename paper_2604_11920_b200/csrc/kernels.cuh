@@ -29,6 +29,7 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
                                                   double* __restrict__ a3, int64_t len, Scalars* sc, double2* partials) {
   __shared__ double2 s_slots[kWarps];
   __shared__ int s_flag;
+  grid_dependency_wait();
   if (VOP != VOP_INIT_U && sc->stop) return;
   Acc<MODE> acc;
   acc.zero();
@@ -91,6 +92,7 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
   }
   lanes_reduce<32, MODE>(acc);
   block_combine<MODE>(acc, s_slots);
+  grid_launch_dependents();
   if (publish_and_ticket(partials, acc.pack(), &sc->ticket[1], &s_flag)) {
     double total = final_sum<MODE>(partials, gridDim.x, s_slots);
     if (threadIdx.x == 0) {

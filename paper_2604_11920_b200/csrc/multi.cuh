@@ -186,10 +186,11 @@ __global__ void __launch_bounds__(kMThreads) k_spmm8(const int64_t* __restrict__
 //   VOP_INIT_U : U = B (B is len x nrhs, nrhs <= 8; missing columns are zero) ; ||b_k||^2
 //   VOP_INIT_VW: V = V * (1/alpha_k) ; W = V ; (X zeroed by the host)
 //   VOP_K4     : as the single-side kernel, with the scalars of side k
+//   VOP_K4_LSMR: LSMR's three-vector update (hbar, x, h) and ||x_k||^2, with the scalars of side k
 template <int MODE, int VOP>
 __global__ void __launch_bounds__(kMThreads) k_vec8(const double* __restrict__ in0, int nrhs, double* __restrict__ a0,
                                                     double* __restrict__ a1, double* __restrict__ a2, int64_t len, Scalars* sc,
-                                                    double2* partials) {
+                                                    double2* partials, double* __restrict__ a3 = nullptr) {
   __shared__ double2 s_slots[kMWarps][kR];
   __shared__ int s_flag;
   const int k = threadIdx.x & 7;
@@ -216,6 +217,22 @@ __global__ void __launch_bounds__(kMThreads) k_vec8(const double* __restrict__ i
       }
     }
     return;
+  } else if (VOP == VOP_K4_LSMR) {  // a0 = V, a1 = H, a2 = X, a3 = Hbar (Fong & Saunders' update with the scalars of side k)
+    if (!stopped) {
+      const double ra = s->ralpha, f1 = s->f1, f2 = s->f2, f3 = s->f3;
+      const bool norm_v = s->norm_v != 0;
+      for (int64_t e = e0; e < total_e; e += stride) {
+        double v = a0[e];
+        if (norm_v) { v = v * ra; a0[e] = v; }
+        const double h = a1[e];
+        const double hb = fma(f1, a3[e], h);
+        a3[e] = hb;
+        const double xn = fma(f2, hb, a2[e]);
+        a2[e] = xn;
+        a1[e] = fma(f3, h, v);
+        acc.mac(xn, xn);
+      }
+    }
   } else if (!stopped) {
     const double ra = s->ralpha, t1 = s->t1, t2 = s->t2, rrho = s->rrho;
     const bool norm_v = s->norm_v != 0;
@@ -244,7 +261,7 @@ __global__ void __launch_bounds__(kMThreads) k_vec8(const double* __restrict__ i
   if (finish_columns<MODE>(bs, partials, &sc->ticket[1], &s_flag, total)) {
     Scalars* t = sc + threadIdx.x;
     if (VOP == VOP_INIT_U) tail_init_u(t, total);
-    else if (!t->stop) tail_k4(t, total);
+    else if (!t->stop) { if (VOP == VOP_K4_LSMR) tail_k4_lsmr(t, total); else tail_k4(t, total); }
     if (threadIdx.x == 0) sc->ticket[1] = 0u;
   }
 }

@@ -16,7 +16,8 @@
 #include "../../include/tomo_lsqr.h"
 #include "build.cuh"
 #include "kernels.cuh"
-#include "stream.cuh"
+#include "wstream.cuh"
+#include "compress.cuh"
 #include "multi.cuh"
 
 using namespace tomo;
@@ -50,8 +51,22 @@ constexpr int kMaxProfileIters = 1 << 16;
 
 }  // namespace
 
+// one direction of the sparse product as the streaming kernel sees it (wstream.cuh): 0 = A over the caller's CSR,
+// 1 = A^T over the CSC copy
+struct Dir {
+  const int64_t* ptr = nullptr;   // starts of the non-empty rows (alias of the CSR / CSC pointer array if no row is empty)
+  int64_t* ptr_own = nullptr;     // ... owned copy when rows had to be compacted away
+  int32_t* rid = nullptr;         // row numbers of the non-empty rows (NULL: identity)
+  int32_t* erows = nullptr;       // rows without elements
+  int nrows = 0, n_empty = 0;     // nrows: non-empty rows
+  const int32_t* idx = nullptr; const void* val = nullptr;
+  int64_t* wE = nullptr; int32_t* wR = nullptr;   // split points of the sms * W warp ranges
+  unsigned char* cidx = nullptr; int64_t* coff = nullptr; int64_t cbytes = 0, heads = 0;  // run-compressed index (FMT 1)
+};
+
 struct tomo_lsqr_s {
   int64_t m = 0, n = 0, nnz = 0;
+  int device = 0;                        // the device the handle was created on; every call checks it is current
   tomo_valtype_t vt = TOMO_VAL_F64;
   // borrowed CSR
   const int64_t* rowptr = nullptr; const int32_t* colind = nullptr; const void* vals = nullptr;
@@ -59,14 +74,16 @@ struct tomo_lsqr_s {
   int64_t* colptr = nullptr; int32_t* rowind = nullptr; void* cvals = nullptr;
   // element split points of the persistent CTAs, per direction
   bool part_dirty = true;
-  int64_t* sE_r = nullptr; int64_t* sE_c = nullptr; int32_t* sR_r = nullptr; int32_t* sR_c = nullptr;
-  CtaRec* cta_rec = nullptr; int SG = 0; int empty_rows = 0, empty_cols = 0;
+  Dir dir[2];
+  CtaRec* cta_rec = nullptr; int SG = 0;
   // work vectors and device state
   double *u = nullptr, *v = nullptr, *w = nullptr, *x = nullptr, *hbar = nullptr;  // w doubles as LSMR's h
   int solver = 0;  // 0 LSQR, 1 LSMR (set per solve)
   // shared-pass multi-RHS state (multi.cuh): len x 8 blocks, eight Scalars, static row partitions
-  double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr; Scalars* msc = nullptr; Scalars* h_msc = nullptr;
+  double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr, *mH = nullptr; Scalars* msc = nullptr; Scalars* h_msc = nullptr;
   int32_t *mpart_r = nullptr, *mpart_c = nullptr; double2* mpartials = nullptr; int MG = 0, multi_shared = 1;
+  bool multi_ready = false;              // every m* allocation succeeded and the partitions were computed
+  PollWord* h_mpoll = nullptr;           // pinned: two slots of eight {itn, istop, stop} words
   cudaGraphExec_t mgexec = nullptr; int mgraph_k = 0, mgraph_mode = -1;
   Scalars* sc = nullptr; double2* part_spmv = nullptr; double2* part_vec = nullptr; int part_cap = 0;
   double *hist_r2 = nullptr, *hist_ar = nullptr; int32_t hist_cap = 0;
@@ -76,7 +93,7 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 96;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 96, pdl = 1, compress = 0;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
@@ -91,44 +108,93 @@ int vec_blocks(const tomo_lsqr_s* h, int64_t len) {
   return (int)std::max<int64_t>(1, std::min<int64_t>(b, (int64_t)h->sms * 16));
 }
 
-// Kernel shapes <elements per chunk, consumer warps, ring stages, L2 prefetch distance>, per accumulation
-// mode (measured on B200, config 1): the double-double sums are instruction-bound, so they take the
-// longer slices (two 256-element rounds per slice, half the per-slice bookkeeping); the plain sums are
-// bandwidth-bound and take the deeper ring, which also leaves ~60 KB of L1 for the gathered vector.
-#ifdef TOMO_CH
-using SCfgFast = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
-using SCfgDD = StreamCfg<TOMO_CH, TOMO_W, TOMO_S, TOMO_PF>;
-#else
-using SCfgFast = StreamCfg<4096, 16, 3, 0>;
-using SCfgDD = StreamCfg<8192, 16, 2, 0>;
+// Kernel shapes <elements per tile, ring stages per warp, warps per CTA> (wstream.cuh), per direction (measured on
+// B200, config 1).  Every warp streams its own contiguous element range through its own ring.  A over the CSR
+// gathers v^ (n doubles, runs of consecutive columns): a 3-stage ring (144 KB) keeps two tiles per warp in
+// flight.  A^T over the CSC gathers u^ (m doubles, short runs): the 2-stage ring (96 KB) leaves ~130 KB of L1 to
+// the gather, which is worth more there than the deeper ring.
+#ifndef TOMO_TILE
+#define TOMO_TILE 256
 #endif
-template <int MODE> struct SCfgOf { using type = SCfgFast; };
-template <> struct SCfgOf<1> { using type = SCfgDD; };
+#ifndef TOMO_NS
+#define TOMO_NS 3
+#endif
+#ifndef TOMO_NS_T
+#define TOMO_NS_T 2
+#endif
+#ifndef TOMO_W
+#define TOMO_W 16
+#endif
+using WC = WCfg<TOMO_TILE, TOMO_NS, TOMO_W>;      // A over the CSR
+using WCT = WCfg<TOMO_TILE, TOMO_NS_T, TOMO_W>;   // A^T over the CSC copy (same tile and warp count: same kind of split points)
+template <bool TR> struct WCOf { using type = WC; };
+template <> struct WCOf<true> { using type = WCT; };
 
-template <int MODE, typename VT, int OP>
-void launch_stream_t(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
-  const int64_t* ptr = transpose ? h->colptr : h->rowptr;
-  const int32_t* idx = transpose ? h->rowind : h->colind;
-  const VT* val = (const VT*)(transpose ? h->cvals : h->vals);
-  const int nrows = (int)(transpose ? h->n : h->m);
-  using SCfg = typename SCfgOf<MODE>::type;
-  auto kern = k_stream<SCfg, MODE, VT, OP>;
-  static bool attr_set = false;  // per instantiation
-  constexpr size_t smem = StreamSmem<SCfg, VT>::kTotal;
-  if (!attr_set) { cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
-  kern<<<h->SG, SCfg::THREADS, smem, st>>>(ptr, idx, val, h->nnz, nrows, transpose ? h->empty_cols : h->empty_rows, x, y,
-                                           transpose ? h->sE_c : h->sE_r, transpose ? h->sR_c : h->sR_r, h->cta_rec, h->sc,
-                                           h->part_spmv);
+template <int MODE, typename VT, int OP, int FMT, bool TR>
+cudaError_t launch_wstream_t(const tomo_lsqr_s* h, const double* x, double* y, cudaStream_t st) {
+  using C = typename WCOf<TR>::type;
+  const Dir& d = h->dir[TR ? 1 : 0];
+  auto kern = k_wstream<C, MODE, VT, OP, FMT>;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)h->SG); cfg.blockDim = dim3(C::THREADS);
+  cfg.dynamicSmemBytes = WSmem<C, VT, FMT>::kTotal; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = (h->pdl && OP != OP_PLAIN) ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, d.ptr, (const int32_t*)d.rid, d.idx, (const VT*)d.val, (const unsigned char*)d.cidx,
+                            (const int64_t*)d.coff, h->nnz, d.nrows, (const int32_t*)d.erows, d.n_empty, x, y,
+                            (const int64_t*)d.wE, (const int32_t*)d.wR, h->cta_rec, h->sc, h->part_spmv);
+}
+
+// The > 48 KB dynamic shared memory opt-in of every k_wstream instantiation, on the CURRENT device (function
+// attributes are per device): called by create, so that a handle on a second GPU works and a refusal is
+// reported at create rather than as an opaque launch error inside a stream capture.
+template <typename C, int MODE, typename VT, int OP, int FMT>
+cudaError_t stream_attr_one() {
+  return cudaFuncSetAttribute(k_wstream<C, MODE, VT, OP, FMT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)WSmem<C, VT, FMT>::kTotal);
+}
+template <int MODE, typename VT, int FMT>
+cudaError_t stream_attr_ops() {
+  cudaError_t e;
+  if ((e = stream_attr_one<WC, MODE, VT, OP_PLAIN, FMT>()) != cudaSuccess) return e;
+  if ((e = stream_attr_one<WC, MODE, VT, OP_K1, FMT>()) != cudaSuccess) return e;
+  if ((e = stream_attr_one<WCT, MODE, VT, OP_PLAIN, FMT>()) != cudaSuccess) return e;
+  if ((e = stream_attr_one<WCT, MODE, VT, OP_K2, FMT>()) != cudaSuccess) return e;
+  return stream_attr_one<WCT, MODE, VT, OP_K2_INIT, FMT>();
+}
+template <typename VT>
+cudaError_t stream_attr_vt() {
+  cudaError_t e;
+  if ((e = stream_attr_ops<0, VT, 0>()) != cudaSuccess) return e;
+  if ((e = stream_attr_ops<1, VT, 0>()) != cudaSuccess) return e;
+  if ((e = stream_attr_ops<0, VT, 1>()) != cudaSuccess) return e;
+  return stream_attr_ops<1, VT, 1>();
+}
+cudaError_t set_kernel_attributes(tomo_valtype_t vt) {
+  return vt == TOMO_VAL_F64 ? stream_attr_vt<double>() : stream_attr_vt<float>();
+}
+
+template <int MODE, typename VT, int OP, int FMT>
+void launch_wstream_dir(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  // K1 runs over the CSR only, K2 / K2_INIT over the CSC only; the plain product runs over either
+  if (OP == OP_K1) launch_wstream_t<MODE, VT, OP_K1, FMT, false>(h, x, y, st);
+  else if (OP == OP_K2) launch_wstream_t<MODE, VT, OP_K2, FMT, true>(h, x, y, st);
+  else if (OP == OP_K2_INIT) launch_wstream_t<MODE, VT, OP_K2_INIT, FMT, true>(h, x, y, st);
+  else if (transpose) launch_wstream_t<MODE, VT, OP_PLAIN, FMT, true>(h, x, y, st);
+  else launch_wstream_t<MODE, VT, OP_PLAIN, FMT, false>(h, x, y, st);
 }
 
 template <int OP>
 void launch_spmv(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  const bool cz = h->compress && h->dir[transpose ? 1 : 0].cidx;
   if (h->vt == TOMO_VAL_F64) {
-    if (h->accumulate) launch_stream_t<1, double, OP>(h, transpose, x, y, st);
-    else launch_stream_t<0, double, OP>(h, transpose, x, y, st);
+    if (h->accumulate) { if (cz) launch_wstream_dir<1, double, OP, 1>(h, transpose, x, y, st); else launch_wstream_dir<1, double, OP, 0>(h, transpose, x, y, st); }
+    else { if (cz) launch_wstream_dir<0, double, OP, 1>(h, transpose, x, y, st); else launch_wstream_dir<0, double, OP, 0>(h, transpose, x, y, st); }
   } else {
-    if (h->accumulate) launch_stream_t<1, float, OP>(h, transpose, x, y, st);
-    else launch_stream_t<0, float, OP>(h, transpose, x, y, st);
+    if (h->accumulate) { if (cz) launch_wstream_dir<1, float, OP, 1>(h, transpose, x, y, st); else launch_wstream_dir<1, float, OP, 0>(h, transpose, x, y, st); }
+    else { if (cz) launch_wstream_dir<0, float, OP, 1>(h, transpose, x, y, st); else launch_wstream_dir<0, float, OP, 0>(h, transpose, x, y, st); }
   }
 }
 
@@ -136,8 +202,14 @@ template <int VOP>
 void launch_vec(const tomo_lsqr_s* h, const double* in0, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st,
                 double* a3 = nullptr) {
   const int g = vec_blocks(h, len);
-  if (h->accumulate) k_vec<1, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
-  else k_vec<0, VOP><<<g, kThreads, 0, st>>>(in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)g); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = (h->pdl && (VOP == VOP_K4 || VOP == VOP_K4_LSMR)) ? 1 : 0;
+  if (h->accumulate) cudaLaunchKernelEx(&cfg, k_vec<1, VOP>, in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
+  else cudaLaunchKernelEx(&cfg, k_vec<0, VOP>, in0, a0, a1, a2, a3, len, h->sc, h->part_vec);
 }
 
 // the vector update that closes an iteration: LSQR's x / w step or LSMR's hbar / x / h step
@@ -149,16 +221,87 @@ void launch_k4(const tomo_lsqr_s* h, cudaStream_t st) {
 tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
   if (!h->part_dirty) return TOMO_OK;
   const int tb = 128;
-  // stream kernel: one persistent CTA per SM, cost-balanced element split points
+  // one persistent CTA per SM, W warp ranges each: cost-balanced element split points at multiples of the tile size
   h->SG = h->sms;
-  const int gs = (h->SG + 1 + tb - 1) / tb;
-  k_stream_partition<<<gs, tb, 0, st>>>(h->rowptr, h->m, h->nnz, h->SG, h->row_cost, h->sE_r, h->sR_r);
-  k_stream_partition<<<gs, tb, 0, st>>>(h->colptr, h->n, h->nnz, h->SG, h->row_cost, h->sE_c, h->sR_c);
+  const int parts = h->SG * WC::W;
+  const int gs = (parts + 1 + tb - 1) / tb;
+  for (int d = 0; d < 2; ++d)
+    k_stream_partition<<<gs, tb, 0, st>>>(h->dir[d].ptr, h->dir[d].nrows, h->nnz, parts, h->row_cost, WC::TILE, h->dir[d].wE, h->dir[d].wR);
   CK(cudaGetLastError());
   h->part_dirty = false;
   return TOMO_OK;
 }
 
+// Rows (d = 0) or columns (d = 1) without elements are compacted away for the streaming kernel and listed.
+tomo_status_t build_dir(tomo_lsqr_s* h, int d, const int64_t* ptr, int64_t nrows, const int32_t* idx, const void* val,
+                        cudaStream_t st) {
+  Dir& D = h->dir[d];
+  D.idx = idx; D.val = val; D.ptr = ptr; D.nrows = (int)nrows; D.n_empty = 0;
+  int* d_cnt = nullptr;
+  CK(cudaMalloc(&d_cnt, sizeof(int)));
+  cudaMemsetAsync(d_cnt, 0, sizeof(int), st);
+  k_count_empty<<<h->sms * 4, 256, 0, st>>>(ptr, nrows, d_cnt);
+  int cnt = 0;
+  cudaError_t e = cudaMemcpyAsync(&cnt, d_cnt, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_cnt);
+  if (e != cudaSuccess) return cuda_fail(e, "count empty rows");
+  if (cnt > 0) {
+    int64_t *flag = nullptr, *pos = nullptr;
+    const int64_t ne = nrows - cnt;
+    e = cudaMalloc(&flag, sizeof(int64_t) * (nrows + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&pos, sizeof(int64_t) * (nrows + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&D.ptr_own, sizeof(int64_t) * (ne + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&D.rid, sizeof(int32_t) * std::max<int64_t>(ne, 1));
+    if (e == cudaSuccess) e = cudaMalloc(&D.erows, sizeof(int32_t) * cnt);
+    if (e == cudaSuccess) {
+      k_flag_nonempty<<<h->sms * 4, 256, 0, st>>>(ptr, nrows, flag);
+      k_exscan<<<1, 1024, 0, st>>>(flag, nrows, pos);
+      k_compact_rows<<<h->sms * 4, 256, 0, st>>>(ptr, nrows, pos, D.ptr_own, D.rid, D.erows);
+      e = cudaGetLastError();
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    cudaFree(flag); cudaFree(pos);
+    if (e != cudaSuccess) return cuda_fail(e, "compact empty rows");
+    D.ptr = D.ptr_own; D.nrows = (int)ne; D.n_empty = cnt;
+  }
+  const int parts = h->sms * WC::W;
+  CK(cudaMalloc(&D.wE, sizeof(int64_t) * (parts + 1)));
+  CK(cudaMalloc(&D.wR, sizeof(int32_t) * (parts + 1)));
+  return TOMO_OK;
+}
+
+}  // namespace
+
+namespace {
+// NEXT-2: the run-compressed index of direction d (compress.cuh), built on first use of option "compress".
+tomo_status_t build_compressed(tomo_lsqr_s* h, int d, cudaStream_t st) {
+  Dir& D = h->dir[d];
+  if (D.cidx || h->nnz == 0) return TOMO_OK;
+  const int64_t ntiles = (h->nnz + WC::TILE - 1) / WC::TILE;
+  int64_t* size = nullptr; int64_t* coff = nullptr; unsigned char* out = nullptr;
+  cudaError_t e = cudaMalloc(&size, sizeof(int64_t) * ntiles);
+  if (e == cudaSuccess) e = cudaMalloc(&coff, sizeof(int64_t) * (ntiles + 1));
+  int64_t total = 0;
+  if (e == cudaSuccess) {
+    k_cz_size<WC::TILE><<<h->sms * 8, 256, 0, st>>>(D.idx, h->nnz, ntiles, size);
+    k_exscan<<<1, 1024, 0, st>>>(size, ntiles, coff);
+    e = cudaMemcpyAsync(&total, coff + ntiles, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&out, (size_t)total + 16);
+  if (e == cudaSuccess) e = cudaMemsetAsync(out, 0, (size_t)total + 16, st);
+  if (e == cudaSuccess) {
+    k_cz_fill<WC::TILE><<<h->sms * 8, 256, 0, st>>>(D.idx, h->nnz, ntiles, coff, out);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  }
+  cudaFree(size);
+  if (e != cudaSuccess) { cudaFree(coff); cudaFree(out); return cuda_fail(e, "build the run-compressed index"); }
+  D.cidx = out; D.coff = coff; D.cbytes = total;
+  D.heads = (total - ntiles * (WC::TILE / 8)) / 4;  // upper bound (includes the 16-byte padding)
+  return TOMO_OK;
+}
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -209,9 +352,10 @@ void free_handle(tomo_lsqr_s* h) {
   for (int i = 0; i < 2; ++i) if (h->ev_poll[i]) cudaEventDestroy(h->ev_poll[i]);
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
   cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
-  cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->msc); cudaFree(h->mpart_r); cudaFree(h->mpart_c);
-  cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
-  cudaFree(h->sE_r); cudaFree(h->sE_c); cudaFree(h->sR_r); cudaFree(h->sR_c); cudaFree(h->cta_rec);
+  cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->mH); cudaFree(h->msc); cudaFree(h->mpart_r); cudaFree(h->mpart_c);
+  cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->h_mpoll) cudaFreeHost(h->h_mpoll); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
+  for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
+  cudaFree(h->cta_rec);
   cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x); cudaFree(h->hbar);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
   cudaFree(h->hist_r2); cudaFree(h->hist_ar); cudaFree(h->bh); cudaFree(h->xh);
@@ -244,7 +388,8 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
 
   tomo_lsqr_s* h = new (std::nothrow) tomo_lsqr_s();
   if (!h) return TOMO_ERR_OOM;
-  h->m = m; h->n = n; h->nnz = nnz; h->vt = vt; h->sms = sms;
+  h->m = m; h->n = n; h->nnz = nnz; h->vt = vt; h->sms = sms; h->device = dev;
+  { cudaError_t ea = set_kernel_attributes(vt); if (ea != cudaSuccess) { delete h; return cuda_fail(ea, "cudaFuncSetAttribute(shared memory opt-in)"); } }
   h->rowptr = d_rowptr; h->colind = d_colind; h->vals = d_vals;
 
   cudaEvent_t e0 = nullptr, e1 = nullptr, e2 = nullptr;
@@ -272,8 +417,6 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     // --- work space ---
     h->part_cap = sms * 32 + 2;  // >= the largest grid of any kernel that publishes partials
 #define ALLOC(p, bytes) if ((e = cudaMalloc(&(p), (bytes))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(work)"); break; }
-    ALLOC(h->sE_r, sizeof(int64_t) * (sms + 1)); ALLOC(h->sE_c, sizeof(int64_t) * (sms + 1));
-    ALLOC(h->sR_r, sizeof(int32_t) * (sms + 1)); ALLOC(h->sR_c, sizeof(int32_t) * (sms + 1));
     ALLOC(h->cta_rec, sizeof(CtaRec) * sms);
     ALLOC(h->u, sizeof(double) * m); ALLOC(h->v, sizeof(double) * n);
     ALLOC(h->w, sizeof(double) * n); ALLOC(h->x, sizeof(double) * n);
@@ -282,19 +425,10 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     ALLOC(h->part_vec, sizeof(double2) * h->part_cap);
 #undef ALLOC
     if ((e = cudaMemsetAsync(h->sc, 0, sizeof(Scalars), st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
-    {  // rows / columns without entries need the (rare) empty-row pass of the stream kernel
-      int* d_cnt = nullptr;
-      if ((e = cudaMalloc(&d_cnt, 2 * sizeof(int))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc"); break; }
-      cudaMemsetAsync(d_cnt, 0, 2 * sizeof(int), st);
-      k_count_empty<<<sms * 4, 256, 0, st>>>(h->rowptr, m, d_cnt);
-      k_count_empty<<<sms * 4, 256, 0, st>>>(h->colptr, n, d_cnt + 1);
-      int cnt[2] = {0, 0};
-      e = cudaMemcpyAsync(cnt, d_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, st);
-      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-      cudaFree(d_cnt);
-      if (e != cudaSuccess) { rc = cuda_fail(e, "count empty rows"); break; }
-      h->empty_rows = cnt[0]; h->empty_cols = cnt[1];
-    }
+    // the two directions of the product as the streaming kernel sees them (rows / columns without entries are
+    // compacted away and listed)
+    if ((rc = build_dir(h, 0, h->rowptr, m, h->colind, h->vals, st)) != TOMO_OK) break;
+    if ((rc = build_dir(h, 1, h->colptr, n, h->rowind, h->cvals, st)) != TOMO_OK) break;
     if ((e = cudaMallocHost(&h->h_sc, sizeof(Scalars))) != cudaSuccess ||
         (e = cudaMallocHost(&h->h_poll, 2 * sizeof(PollWord))) != cudaSuccess) { rc = cuda_fail(e, "cudaMallocHost"); break; }
     for (int i = 0; i < 2; ++i)
@@ -393,7 +527,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
   const int k = h->check_every;
   const int chunks = max_iters > 0 ? (max_iters + k - 1) / k : 0;
   if (profile) {
-    const size_t need = (size_t)std::min(max_iters, kMaxProfileIters) * 4;
+    const size_t need = (size_t)std::min((int64_t)chunks * k, (int64_t)kMaxProfileIters) * 4;
     while (h->prof_ev.size() < need) {
       cudaEvent_t e; CK(cudaEventCreate(&e)); h->prof_ev.push_back(e);
     }
@@ -454,8 +588,17 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
   return TOMO_OK;
 }
 
+// a handle lives on the device it was created on: that device must be the current one
+tomo_status_t check_device(const tomo_lsqr_s* h) {
+  if (!h) return TOMO_ERR_INVALID_ARG;
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  return dev == h->device ? TOMO_OK : TOMO_ERR_INVALID_ARG;
+}
+
 tomo_status_t check_solve_args(tomo_lsqr_s* h, double damp, double atol, double btol, int32_t max_iters) {
   if (!h) return TOMO_ERR_INVALID_ARG;
+  { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
   if (bad_param(damp) || bad_param(atol) || bad_param(btol) || max_iters < 0) return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
 }
@@ -486,21 +629,33 @@ extern "C" tomo_status_t tomo_lsmr_solve(tomo_lsqr_t h, const double* d_b, doubl
   return rc;
 }
 
-extern "C" tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
-                                              int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream) {
+namespace {
+tomo_status_t solve_host_any(tomo_lsqr_s* h, int solver, const double* h_b, double damp, double atol, double btol,
+                             int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, cudaStream_t st) {
   tomo_status_t rc = check_solve_args(h, damp, atol, btol, max_iters);
   if (rc != TOMO_OK) return rc;
   if (!h_b || !h_x) return TOMO_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
   if (!h->bh) CK(cudaMalloc(&h->bh, sizeof(double) * h->m));
   if (!h->xh) CK(cudaMalloc(&h->xh, sizeof(double) * h->n));
   CK(cudaMemcpyAsync(h->bh, h_b, sizeof(double) * h->m, cudaMemcpyHostToDevice, st));
-  h->solver = 0;
+  h->solver = solver;
   rc = solve_device(h, h->bh, damp, atol, btol, max_iters, h->xh, res, nullptr, nullptr, st);
+  h->solver = 0;
   if (rc != TOMO_OK) return rc;
   CK(cudaMemcpyAsync(h_x, h->xh, sizeof(double) * h->n, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
   return TOMO_OK;
+}
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
+                                              int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream) {
+  return solve_host_any(h, 0, h_b, damp, atol, btol, max_iters, h_x, res, (cudaStream_t)cuda_stream);
+}
+
+extern "C" tomo_status_t tomo_lsmr_solve_host(tomo_lsqr_t h, const double* h_b, double damp, double atol, double btol,
+                                              int32_t max_iters, double* h_x, tomo_lsqr_result_t* res, void* cuda_stream) {
+  return solve_host_any(h, 1, h_b, damp, atol, btol, max_iters, h_x, res, (cudaStream_t)cuda_stream);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -539,38 +694,73 @@ void launch_spmm(const tomo_lsqr_s* h, bool transpose, const double* X, double* 
 }
 
 template <int VOP>
-void launch_vec8(const tomo_lsqr_s* h, const double* in0, int nrhs, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st) {
+void launch_vec8(const tomo_lsqr_s* h, const double* in0, int nrhs, double* a0, double* a1, double* a2, int64_t len, cudaStream_t st,
+                 double* a3 = nullptr) {
   const int g = (int)std::max<int64_t>(1, std::min<int64_t>((len * kR + kMThreads - 1) / kMThreads, (int64_t)h->MG));
-  if (h->accumulate) k_vec8<1, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials);
-  else k_vec8<0, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials);
+  if (h->accumulate) k_vec8<1, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials, a3);
+  else k_vec8<0, VOP><<<g, kMThreads, 0, st>>>(in0, nrhs, a0, a1, a2, len, h->msc, h->mpartials, a3);
 }
 
 void enqueue_multi_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
   launch_spmm<OP_K1>(h, false, h->mV, h->mU, st);
   launch_spmm<OP_K2>(h, true, h->mU, h->mV, st);
-  launch_vec8<VOP_K4>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st);
+  if (h->solver == 1) launch_vec8<VOP_K4_LSMR>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st, h->mH);
+  else launch_vec8<VOP_K4>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st);
+}
+
+// Work space of the block solve, allocated on first use.  All-or-nothing: the pointers are committed to the
+// handle only after every allocation and the partition kernels have succeeded, so a transient out-of-memory
+// leaves the handle as it was.
+tomo_status_t ensure_multi(tomo_lsqr_s* h, cudaStream_t st) {
+  if (h->multi_ready) return TOMO_OK;
+  const int64_t m = h->m, n = h->n;
+  const int MG = h->sms * 8;
+  double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr, *mH = nullptr;
+  Scalars *msc = nullptr, *h_msc = nullptr; PollWord* h_mpoll = nullptr;
+  int32_t *pr = nullptr, *pc = nullptr; double2* mp = nullptr;
+  cudaError_t e = cudaSuccess;
+  do {
+    if ((e = cudaMalloc(&mU, sizeof(double) * m * kR)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&mV, sizeof(double) * n * kR)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&mW, sizeof(double) * n * kR)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&mX, sizeof(double) * n * kR)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&mH, sizeof(double) * n * kR)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&msc, sizeof(Scalars) * kR)) != cudaSuccess) break;
+    if ((e = cudaMallocHost(&h_msc, sizeof(Scalars) * kR)) != cudaSuccess) break;
+    if ((e = cudaMallocHost(&h_mpoll, sizeof(PollWord) * kR * 2)) != cudaSuccess) break;
+    if ((e = cudaMalloc(&pr, sizeof(int32_t) * (MG + 1))) != cudaSuccess) break;
+    if ((e = cudaMalloc(&pc, sizeof(int32_t) * (MG + 1))) != cudaSuccess) break;
+    if ((e = cudaMalloc(&mp, sizeof(double2) * kR * MG)) != cudaSuccess) break;
+    const int tb = 128, gb = (MG + 1 + tb - 1) / tb;
+    k_partition<<<gb, tb, 0, st>>>(h->rowptr, m, MG, 16, 1, pr);
+    k_partition_fix<<<1, 32, 0, st>>>(MG, pr);
+    k_partition<<<gb, tb, 0, st>>>(h->colptr, n, MG, 16, 1, pc);
+    k_partition_fix<<<1, 32, 0, st>>>(MG, pc);
+    if ((e = cudaGetLastError()) != cudaSuccess) break;
+    e = cudaStreamSynchronize(st);
+  } while (0);
+  if (e != cudaSuccess) {
+    cudaFree(mU); cudaFree(mV); cudaFree(mW); cudaFree(mX); cudaFree(mH); cudaFree(msc); cudaFree(pr); cudaFree(pc); cudaFree(mp);
+    if (h_msc) cudaFreeHost(h_msc);
+    if (h_mpoll) cudaFreeHost(h_mpoll);
+    return cuda_fail(e, "block-solve work space");
+  }
+  h->mU = mU; h->mV = mV; h->mW = mW; h->mX = mX; h->mH = mH; h->msc = msc; h->h_msc = h_msc; h->h_mpoll = h_mpoll;
+  h->mpart_r = pr; h->mpart_c = pc; h->mpartials = mp; h->MG = MG;
+  h->multi_ready = true;
+  return TOMO_OK;
 }
 
 // Eight recurrences sharing every pass over A and A^T (multi.cuh).  nrhs < 8 is padded with zero columns.
-tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int32_t nrhs, const double* d_B, double damp, double atol, double btol,
+// solver: 0 LSQR, 1 LSMR (per-side scalars either way).
+tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int solver, int32_t nrhs, const double* d_B, double damp, double atol, double btol,
                                  int32_t max_iters, double* d_X, tomo_lsqr_result_t* res, cudaStream_t st) {
   const int64_t m = h->m, n = h->n;
-  if (!h->mU) {
-    CK(cudaMalloc(&h->mU, sizeof(double) * m * kR)); CK(cudaMalloc(&h->mV, sizeof(double) * n * kR));
-    CK(cudaMalloc(&h->mW, sizeof(double) * n * kR)); CK(cudaMalloc(&h->mX, sizeof(double) * n * kR));
-    CK(cudaMalloc(&h->msc, sizeof(Scalars) * kR)); CK(cudaMallocHost(&h->h_msc, sizeof(Scalars) * kR));
-    h->MG = h->sms * 8;
-    CK(cudaMalloc(&h->mpart_r, sizeof(int32_t) * (h->MG + 1))); CK(cudaMalloc(&h->mpart_c, sizeof(int32_t) * (h->MG + 1)));
-    CK(cudaMalloc(&h->mpartials, sizeof(double2) * kR * h->MG));
-    const int tb = 128, gb = (h->MG + 1 + tb - 1) / tb;
-    k_partition<<<gb, tb, 0, st>>>(h->rowptr, m, h->MG, 16, 1, h->mpart_r);
-    k_partition_fix<<<1, 32, 0, st>>>(h->MG, h->mpart_r);
-    k_partition<<<gb, tb, 0, st>>>(h->colptr, n, h->MG, 16, 1, h->mpart_c);
-    k_partition_fix<<<1, 32, 0, st>>>(h->MG, h->mpart_c);
-    CK(cudaGetLastError());
-  }
+  { tomo_status_t rc = ensure_multi(h, st); if (rc != TOMO_OK) return rc; }
+  h->solver = solver;
   const int k = h->check_every;
-  if (h->use_graph && !(h->mgexec && h->mgraph_k == k && h->mgraph_mode == h->accumulate)) {
+  const int gkey = h->accumulate + 2 * solver;
+  if (h->use_graph && !(h->mgexec && h->mgraph_k == k && h->mgraph_mode == gkey)) {
     if (h->mgexec) { cudaGraphExecDestroy(h->mgexec); h->mgexec = nullptr; }
     cudaGraph_t g = nullptr;
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed));
@@ -580,31 +770,61 @@ tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int32_t nrhs, const double* d_B
     e = cudaGraphInstantiate(&h->mgexec, g, 0);
     cudaGraphDestroy(g);
     if (e != cudaSuccess) { h->mgexec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
-    h->mgraph_k = k; h->mgraph_mode = h->accumulate;
+    h->mgraph_k = k; h->mgraph_mode = gkey;
   }
   Scalars* hs = h->h_msc;
   memset(hs, 0, sizeof(Scalars) * kR);
-  for (int r = 0; r < kR; ++r) { hs[r].damp = damp; hs[r].atol = atol; hs[r].btol = btol; hs[r].max_iters = max_iters; hs[r].cs2 = -1.0; }
+  for (int r = 0; r < kR; ++r) {
+    hs[r].damp = damp; hs[r].atol = atol; hs[r].btol = btol; hs[r].max_iters = max_iters; hs[r].cs2 = -1.0; hs[r].solver = solver;
+  }
   CK(cudaMemcpyAsync(h->msc, hs, sizeof(Scalars) * kR, cudaMemcpyHostToDevice, st));
   CK(cudaMemsetAsync(h->mX, 0, sizeof(double) * n * kR, st));
   CK(cudaMemsetAsync(h->mV, 0, sizeof(double) * n * kR, st));
   CK(cudaMemsetAsync(h->mW, 0, sizeof(double) * n * kR, st));
+  if (solver == 1) CK(cudaMemsetAsync(h->mH, 0, sizeof(double) * n * kR, st));
   launch_vec8<VOP_INIT_U>(h, d_B, nrhs, h->mU, nullptr, nullptr, m, st);
   launch_spmm<OP_K2_INIT>(h, true, h->mU, h->mV, st);
   launch_vec8<VOP_INIT_VW>(h, nullptr, kR, h->mV, h->mW, nullptr, n, st);
   CK(cudaGetLastError());
   h->kernels_enqueued += 3;
+  const bool profile = h->profile != 0;
+  const bool graph = h->use_graph && !profile;
   const int chunks = max_iters > 0 ? (max_iters + k - 1) / k : 0;
-  for (int c = 0; c < chunks; ++c) {
-    if (h->use_graph) CK(cudaGraphLaunch(h->mgexec, st));
-    else { for (int i = 0; i < k; ++i) enqueue_multi_iteration(h, st); CK(cudaGetLastError()); }
+  if (profile) {
+    const size_t need = (size_t)std::min((int64_t)chunks * k, (int64_t)kMaxProfileIters) * 4;
+    while (h->prof_ev.size() < need) { cudaEvent_t e; CK(cudaEventCreate(&e)); h->prof_ev.push_back(e); }
+  }
+  int it_enq = 0;
+  bool stopped = false;
+  for (int c = 0; c < chunks && !stopped; ++c) {
+    const int slot = c & 1;
+    if (graph) CK(cudaGraphLaunch(h->mgexec, st));
+    else {
+      for (int i = 0; i < k; ++i, ++it_enq) {
+        const bool pe = profile && it_enq < kMaxProfileIters;
+        if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 0], st);
+        launch_spmm<OP_K1>(h, false, h->mV, h->mU, st);
+        if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 1], st);
+        launch_spmm<OP_K2>(h, true, h->mU, h->mV, st);
+        if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 2], st);
+        if (solver == 1) launch_vec8<VOP_K4_LSMR>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st, h->mH);
+        else launch_vec8<VOP_K4>(h, nullptr, kR, h->mV, h->mW, h->mX, h->n, st);
+        if (pe) cudaEventRecord(h->prof_ev[4 * it_enq + 3], st);
+      }
+      CK(cudaGetLastError());
+    }
     h->kernels_enqueued += 3.0 * k;
-    // poll: the eight {itn, istop, stop} words; stop when every side has stopped
-    CK(cudaMemcpy2DAsync(h->h_msc, sizeof(Scalars), h->msc, sizeof(Scalars), sizeof(Scalars), kR, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    bool all = true;
-    for (int r = 0; r < kR; ++r) all = all && (h->h_msc[r].stop != 0);
-    if (all) break;
+    // poll the eight {itn, istop, stop} words one replay behind the one being enqueued (as solve_device does):
+    // the device never idles on the host; replays after every side has stopped are empty launches
+    CK(cudaMemcpy2DAsync(h->h_mpoll + (size_t)slot * kR, sizeof(PollWord), &h->msc->itn, sizeof(Scalars), sizeof(PollWord), kR,
+                         cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(h->ev_poll[slot], st));
+    if (c >= 1) {
+      CK(cudaEventSynchronize(h->ev_poll[slot ^ 1]));
+      bool all = true;
+      for (int r = 0; r < kR; ++r) all = all && (h->h_mpoll[(size_t)(slot ^ 1) * kR + r].stop != 0);
+      if (all) stopped = true;
+    }
   }
   CK(cudaMemcpyAsync(h->h_msc, h->msc, sizeof(Scalars) * kR, cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpy2DAsync(d_X, sizeof(double) * nrhs, h->mX, sizeof(double) * kR, sizeof(double) * nrhs, n, cudaMemcpyDeviceToDevice, st));
@@ -615,26 +835,41 @@ tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int32_t nrhs, const double* d_B
       res[r].itn = q.itn; res[r].istop = q.istop; res[r].r1norm = q.r1norm; res[r].r2norm = q.r2norm;
       res[r].arnorm = q.arnorm; res[r].anorm = q.anorm; res[r].acond = q.acond; res[r].xnorm = q.xnorm;
     }
+  if (profile) {
+    h->k1_ms = h->k2_ms = h->k4_ms = 0; h->k_launches = 0;
+    int itn_max = 0;
+    for (int r = 0; r < kR; ++r) itn_max = std::max(itn_max, (int)h->h_msc[r].itn);
+    const int cnt = std::min<int>(std::min<int>(itn_max, it_enq), kMaxProfileIters);
+    for (int i = 0; i < cnt; ++i) {
+      float a = 0, b = 0, c4 = 0;
+      cudaEventElapsedTime(&a, h->prof_ev[4 * i], h->prof_ev[4 * i + 1]);
+      cudaEventElapsedTime(&b, h->prof_ev[4 * i + 1], h->prof_ev[4 * i + 2]);
+      cudaEventElapsedTime(&c4, h->prof_ev[4 * i + 2], h->prof_ev[4 * i + 3]);
+      h->k1_ms += a; h->k2_ms += b; h->k4_ms += c4;
+    }
+    h->k_launches = cnt;
+  }
   return TOMO_OK;
 }
 
-}  // namespace
-
-extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
-                                               double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
-                                               void* cuda_stream) {
+tomo_status_t solve_multi_any(tomo_lsqr_s* h, int solver, int32_t nrhs, const double* d_B, double damp, double atol, double btol,
+                              int32_t max_iters, double* d_X, tomo_lsqr_result_t* res, cudaStream_t st) {
   tomo_status_t rc = check_solve_args(h, damp, atol, btol, max_iters);
   if (rc != TOMO_OK) return rc;
   if (nrhs < 1 || nrhs > 8 || !d_B || !d_X) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_B) || !is_device_ptr(d_X)) return TOMO_ERR_NOT_DEVICE_PTR;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (h->multi_shared) return solve_multi_shared(h, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, st);
+  if (h->multi_shared) {
+    rc = solve_multi_shared(h, solver, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, st);
+    h->solver = 0;
+    return rc;
+  }
   if (!h->bh) CK(cudaMalloc(&h->bh, sizeof(double) * h->m));
   if (!h->xh) CK(cudaMalloc(&h->xh, sizeof(double) * h->n));
   for (int r = 0; r < nrhs; ++r) {
     k_col_gather<<<vec_blocks(h, h->m), kThreads, 0, st>>>(d_B, nrhs, r, h->m, h->bh);
-    h->solver = 0;
+    h->solver = solver;
     rc = solve_device(h, h->bh, damp, atol, btol, max_iters, h->xh, res ? res + r : nullptr, nullptr, nullptr, st);
+    h->solver = 0;
     if (rc != TOMO_OK) return rc;
     k_col_scatter<<<vec_blocks(h, h->n), kThreads, 0, st>>>(h->xh, nrhs, r, h->n, d_X);
   }
@@ -643,11 +878,27 @@ extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, cons
   return TOMO_OK;
 }
 
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
+                                               double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
+                                               void* cuda_stream) {
+  return solve_multi_any(h, 0, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, (cudaStream_t)cuda_stream);
+}
+
+extern "C" tomo_status_t tomo_lsmr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
+                                               double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
+                                               void* cuda_stream) {
+  return solve_multi_any(h, 1, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, (cudaStream_t)cuda_stream);
+}
+
 extern "C" tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const double* d_in, double* d_out, void* cuda_stream) {
   if (!h || !d_in || !d_out || (transpose != 0 && transpose != 1)) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_in) || !is_device_ptr(d_out)) return TOMO_ERR_NOT_DEVICE_PTR;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  tomo_status_t rc = rebuild_partitions(h, st);
+  tomo_status_t rc = check_device(h);
+  if (rc != TOMO_OK) return rc;
+  rc = rebuild_partitions(h, st);
   if (rc != TOMO_OK) return rc;
   launch_spmv<OP_PLAIN>(h, transpose != 0, d_in, d_out, st);
   CK(cudaGetLastError());
@@ -657,6 +908,7 @@ extern "C" tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const doub
 
 extern "C" tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_rowind, void* d_cvals, void* cuda_stream) {
   if (!h) return TOMO_ERR_INVALID_ARG;
+  { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t vb = h->vt == TOMO_VAL_F64 ? sizeof(double) : sizeof(float);
   if (d_colptr) CK(cudaMemcpyAsync(d_colptr, h->colptr, sizeof(int64_t) * (h->n + 1), cudaMemcpyDeviceToDevice, st));
@@ -670,10 +922,18 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   if (!h || !key) return TOMO_ERR_INVALID_ARG;
   const std::string k(key);
   if (k == "check_every") { if (value < 1 || value > 100000) return TOMO_ERR_INVALID_ARG; h->check_every = (int)value; }
-  else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; if (h->accumulate != (int)value) h->part_dirty = true; h->accumulate = (int)value; }
+  else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
   else if (k == "multi_shared") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->multi_shared = (int)value; }
+  else if (k == "compress") {
+    if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG;
+    { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
+    if (value == 1) for (int d = 0; d < 2; ++d) { tomo_status_t rc = build_compressed(h, d, nullptr); if (rc != TOMO_OK) return rc; }
+    if (h->compress != (int)value && h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    h->compress = (int)value;
+  }
+  else if (k == "pdl") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; if (h->pdl != (int)value && h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; } h->pdl = (int)value; }
   else if (k == "row_cost") { if (value < 0 || value > 4096) return TOMO_ERR_INVALID_ARG; if (h->row_cost != (int)value) h->part_dirty = true; h->row_cost = (int)value; }
   else return TOMO_ERR_INVALID_ARG;
   return TOMO_OK;
@@ -687,6 +947,8 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "transpose_ms") *out = h->transpose_ms;
   else if (k == "csc_bytes") *out = (double)h->nnz * (4.0 + vb) + 8.0 * (double)(h->n + 1);
   else if (k == "scratch_bytes") *out = h->scratch_bytes;
+  else if (k == "compress_bytes_rows") *out = (double)h->dir[0].cbytes + 8.0 * (double)((h->nnz + WC::TILE - 1) / WC::TILE + 1);
+  else if (k == "compress_bytes_cols") *out = (double)h->dir[1].cbytes + 8.0 * (double)((h->nnz + WC::TILE - 1) / WC::TILE + 1);
   else if (k == "blocks_rows" || k == "blocks_cols") *out = (double)h->SG;
   else if (k == "k1_ms") *out = h->k1_ms;
   else if (k == "k2_ms") *out = h->k2_ms;

@@ -17,11 +17,25 @@ _pool: ProcessPoolExecutor | None = None
 _jobs: dict[tuple, Future] = {}
 
 
+def _available_ram() -> float:
+    try:
+        import psutil
+        return float(psutil.virtual_memory().available)
+    except Exception:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return 1024.0 * float(line.split()[1])
+    return 0.0
+
+
 def _run(cfg: int, rhs: int, mode: int, damp: float, atol: float, btol: float, max_iters: int, snapshots: tuple,
          f32_values: bool = False, solver: str = "lsqr"):
     import oracle
     import tomogen
     s = tomogen.System(cfg)
+    need = 13.0 * s.dims.nnz + 64.0 * (s.dims.m + s.dims.n)  # CSR (12 B/nnz) + vectors + slack
+    if cfg == 2 and _available_ram() < need + 8e9:
+        return dict(skipped=f"host RAM: {_available_ram() / 1e9:.0f} GB available, the config-2 CSR needs {need / 1e9:.0f} GB")
     rp, ci, va = s.csr()
     if f32_values:  # the fp32-storage path: the oracle sees the same rounded values, widened to fp64
         va = va.astype(np.float32).astype(np.float64)
@@ -49,11 +63,15 @@ def _all_jobs():
         ("cfg1_dd_f32_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), True),
         # config 1 by LSMR (NEXT-1)
         ("cfg1_lsmr_dd_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), False, "lsmr"),
-        # config 3: columns 0 and 7 of the 8 right-hand sides
-        ("cfg3_dd_rhs0",): (3, 0, oracle.DD, d1, 0.0, 0.0, 50, ()),
-        ("cfg3_dd_rhs7",): (3, 7, oracle.DD, d1, 0.0, 0.0, 50, ()),
         # config 4: skewed system, 100 iterations with x_50 as a snapshot
         ("cfg4_dd_100",): (4, 0, oracle.DD, d4, 0.0, 0.0, 100, (50,)),
+        # config 2 (3.7e9 nnz): x_5 of the dd oracle at full size (~45 GB of host RAM, ~25 s per iteration)
+        ("cfg2_dd_5",): (2, 0, oracle.DD, tomogen.System(2).damp, 0.0, 0.0, 5, (1, 2)),
+        # config 3: every one of the 8 right-hand sides, 100 iterations as BASELINE.json states (x_50 as a snapshot)
+        **{(f"cfg3_dd_rhs{r}",): (3, r, oracle.DD, d1, 0.0, 0.0, 100, (50,)) for r in range(8)},
+        # config 1 by LSMR on the block path (columns 0 and 5 of config 3's right-hand sides)
+        ("cfg3_lsmr_dd_rhs0",): (3, 0, oracle.DD, d1, 0.0, 0.0, 50, (), False, "lsmr"),
+        ("cfg3_lsmr_dd_rhs5",): (3, 5, oracle.DD, d1, 0.0, 0.0, 50, (), False, "lsmr"),
     }
 
 
@@ -61,9 +79,14 @@ def start():
     global _pool
     if _pool is not None:
         return
-    workers = max(1, min(7, (os.cpu_count() or 2) - 1))
+    jobs = _all_jobs()
+    # one worker per job if the host has the cores and the memory (a config-1-sized job holds ~3 GB, the
+    # config-2 job ~50 GB); the long jobs are submitted first
+    by_ram = int(max(1.0, (_available_ram() - 60e9) / 4e9))
+    workers = max(1, min(len(jobs), (os.cpu_count() or 2) - 1, by_ram))
     _pool = ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn"))
-    for key, args in _all_jobs().items():
+    order = sorted(jobs.items(), key=lambda kv: -(kv[1][6] * (20 if kv[1][0] == 2 else 1)))
+    for key, args in order:
         _jobs[key] = _pool.submit(_run, *args)
 
 

@@ -31,3 +31,18 @@ def test_two_gloo_ranks_aggregate_like_the_bench(tmp_path):
     line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
     d = json.loads(line)
     assert d == dict(ms=150.0, its=601, launches=1806.0, world=2)
+
+
+def test_bench_gpus_2_self_launches_its_ranks():
+    """`python bench.py --gpus 2` as the driver invokes it (no torchrun around it) must start its own two ranks;
+    here with the test-only stub step (no GPU): one JSON line, n_gpus = 2, max-over-ranks time, summed units."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3", "--stub-step"],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["stub"] is True and d["n_gpus"] == 2 and d["value"] is None
+    assert d["ms_per_step"] == 20.0 / 3 and d["stub_iterations"] == 42 and d["stub_launches"] == 126.0

@@ -56,11 +56,70 @@ def test_dd_spmv_is_correctly_rounded_exact_sum():
     x = np.ones(n) + 1e-7 * rng.standard_normal(n)
     A = sp.csr_matrix(D)
     y = oracle.spmv(*csr_args(A), x, oracle.DD)
-    yt = oracle.spmv_t(*csr_args(A), np.ones(m) + 1e-7 * rng.standard_normal(m), oracle.DD)
     for i in range(m):
         exact = sum(Fraction(D[i, j]) * Fraction(x[j]) for j in range(n))
         assert y[i] == float(exact)  # float(Fraction) rounds to nearest
-    assert np.isfinite(yt).all()
+    # the transposed product (a scatter with one (hi, lo) pair per column) on sums that cancel just as
+    # badly: the transpose of the same construction, so every COLUMN sum loses ~9 digits; a scatter that
+    # dropped or mis-paired the low word would be off by ~1e-9 relative here
+    Dt = np.ascontiguousarray(D.T)          # n x m: column i of Dt is row i of D
+    At = sp.csr_matrix(Dt)
+    yt = oracle.spmv_t(*csr_args(At), x, oracle.DD)   # (Dt)^T x = D x, computed by the scatter
+    for i in range(m):
+        exact = sum(Fraction(Dt[j, i]) * Fraction(x[j]) for j in range(n))
+        assert yt[i] == float(exact)
+    assert np.array_equal(yt, y)            # both routes give the one correctly rounded value
+    u = np.ones(m) + 1e-7 * rng.standard_normal(m)
+    yu = oracle.spmv_t(*csr_args(A), u, oracle.DD)
+    for j in range(n):
+        exact = sum(Fraction(D[i, j]) * Fraction(u[i]) for i in range(m))
+        assert yu[j] == float(exact)
+
+
+def test_fused_axpy_terms_and_norms_are_exact_in_dd_mode():
+    """spmv / spmv_t with c != 0 (u <- A v - alpha u, v <- A^T u - beta v: the fused term enters the same
+    (hi, lo) sum and the total is rounded once) and the dd norms, pinned through the first iteration of the
+    Stepper against exact rational arithmetic.  A dropped or separately rounded -alpha*u_i / -beta*v_j
+    term, a wrong sign or a norm that is not the rounded exact sum changes the last bits checked here."""
+    rng = np.random.default_rng(15)
+    m, n = 14, 9
+    D = rng.standard_normal((m, n)) * (rng.random((m, n)) < 0.6)
+    D[0, :] = 0.0
+    D[0, 0] = 1.0  # keep every column and row non-trivial enough
+    A = sp.csr_matrix(D)
+    A.sort_indices()
+    b = rng.standard_normal(m)
+    st = oracle.Stepper(*csr_args(A), b, damp=0.3, max_iters=3, mode=oracle.DD)
+    F = Fraction
+
+    def rsum(terms):  # correctly rounded exact sum
+        return float(sum(terms, F(0)))
+
+    # state after init: u = b/||b||, v = A^T u / alpha (both rounded as the algorithm states)
+    beta1 = np.sqrt(rsum(F(t) * F(t) for t in b))
+    u0 = b * (1.0 / beta1)
+    assert np.array_equal(st.vec("u"), u0)
+    vh = np.array([rsum(F(D[i, j]) * F(u0[i]) for i in range(m)) for j in range(n)])
+    alpha1 = np.sqrt(rsum(F(t) * F(t) for t in vh))
+    v0 = vh * (1.0 / alpha1)
+    assert np.array_equal(st.vec("v"), v0)
+    sc = st.scalars()
+    assert sc["alpha"] == alpha1 and sc["beta"] == beta1
+    # one iteration: u^ = A v - alpha u, beta, u = u^/beta ; v^ = A^T u - beta v, alpha, v = v^/alpha
+    st.step()
+    uh = np.array([rsum([F(-alpha1) * F(u0[i])] + [F(D[i, j]) * F(v0[j]) for j in range(n)]) for i in range(m)])
+    beta2 = np.sqrt(rsum(F(t) * F(t) for t in uh))
+    u1 = uh * (1.0 / beta2)
+    assert np.array_equal(st.vec("u"), u1)
+    vh2 = np.array([rsum([F(-beta2) * F(v0[j])] + [F(D[i, j]) * F(u1[i]) for i in range(m)]) for j in range(n)])
+    alpha2 = np.sqrt(rsum(F(t) * F(t) for t in vh2))
+    assert np.array_equal(st.vec("v"), vh2 * (1.0 / alpha2))
+    sc = st.scalars()
+    assert sc["alpha"] == alpha2 and sc["beta"] == beta2
+    # plain mode takes the same terms in fp64 with the fused term LAST (fma(c, y_i, s)): pinned to rounding
+    sp_ = oracle.Stepper(*csr_args(A), b, damp=0.3, max_iters=3, mode=oracle.PLAIN)
+    sp_.step()
+    assert rel(sp_.vec("u"), u1) < 1e-14 and rel(sp_.vec("v"), vh2 * (1.0 / alpha2)) < 1e-13
 
 
 def test_adjoint_identity(cfg0):
