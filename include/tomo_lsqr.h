@@ -77,6 +77,17 @@ typedef struct {
 tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr,
                                const int32_t* d_colind, const void* d_vals, tomo_valtype_t vt, void* cuda_stream);
 
+/* NEXT-4: value-only refresh.  The outer Gauss-Newton loop of the inversion
+ * re-evaluates G on the same rays and solves again: the sparsity pattern, hence the CSC permutation, the split
+ * points and the compressed index, stay; only the values change.  d_vals: device array [nnz] of the handle's value
+ * type, in CSR order of the pattern given at create, finite, 16-byte aligned; it may be the array given at create
+ * (overwritten in place by the caller) or another one, which then REPLACES it as the borrowed value array (same
+ * lifetime rule).  The first call records the CSR -> CSC permutation (one replay of the transpose passes, 4 bytes
+ * per nonzero, 8 if nnz >= 2^32); every call then costs one pass over the values ("update_ms" in get_info).
+ * Results of later solves are bitwise those of a handle created from scratch on the new values.
+ * Errors: TOMO_ERR_BAD_CSR (a non-finite value; the handle is unchanged), INVALID_ARG, NOT_DEVICE_PTR, OOM, CUDA. */
+tomo_status_t tomo_lsqr_update_values(tomo_lsqr_t h, const void* d_vals, void* cuda_stream);
+
 /* a1-a7: LSQR on (A, b, damp) from x_0 = 0 until a stopping test fires or max_iters iterations.
  * d_b fp64[m], d_x fp64[n].  damp, atol, btol >= 0 and finite; max_iters >= 0 (0: x = 0, istop = 7).
  * h_r2norm_hist / h_arnorm_hist: NULL or host fp64[max_iters]; entry k-1 = r2norm / arnorm after
@@ -141,10 +152,12 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *                          prologue of a kernel (barrier set-up, split points, first bulk copies) overlaps the
  *                          tail of the previous one; never changes results
  *   "row_cost"    c >= 0   weight of a row, in elements, in the cost-balanced element split of the
- *                          persistent CTAs (default 96); changes the summation order only */
+ *                          warp ranges (default 320: a row end costs about as much as 320 streamed elements, measured on B200); changes the summation order only */
 tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value);
 
-/* Read-outs (host double): "create_ms", "transpose_ms", "csc_bytes", "scratch_bytes", "blocks_rows",
+/* Read-outs (host double): "create_ms" (whole create call, CUDA events), "transpose_ms" (its transpose section
+ * including the allocation of the CSC arrays and scratch), "transpose_kernels_ms" (the transpose kernels alone),
+ * "update_ms" (the last tomo_lsqr_update_values pass), "csc_bytes", "scratch_bytes", "blocks_rows",
  * "blocks_cols", "compress_bytes_rows" / "compress_bytes_cols" (bytes of the run-compressed index of each direction,
  * 0 before "compress" was set), and after a solve with "profile"=1: "k1_ms", "k2_ms", "k4_ms" (summed CUDA-event time of
  * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each);

@@ -23,7 +23,7 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
     "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
-    "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv",
+    "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
 )
 
@@ -61,6 +61,7 @@ def load() -> ctypes.CDLL:
     lib.tomo_lsqr_solve_multi.argtypes = [vp, i32, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
     lib.tomo_lsmr_solve_multi.argtypes = lib.tomo_lsqr_solve_multi.argtypes
     lib.tomo_lsqr_spmv.argtypes = [vp, ci, vp, vp, vp]
+    lib.tomo_lsqr_update_values.argtypes = [vp, vp, vp]
     lib.tomo_lsqr_get_csc.argtypes = [vp, vp, vp, vp, vp]
     lib.tomo_lsqr_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.tomo_lsqr_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(f64)]
@@ -166,6 +167,12 @@ def tomo_lsqr_spmv(h, transpose, d_in, d_out, stream=None) -> None:
         raise TomoError(st, "tomo_lsqr_spmv")
 
 
+def tomo_lsqr_update_values(h, d_vals, stream=None) -> None:
+    st = load().tomo_lsqr_update_values(h, _ptr(d_vals), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_update_values")
+
+
 def tomo_lsqr_get_csc(h, d_colptr, d_rowind, d_cvals, stream=None) -> None:
     st = load().tomo_lsqr_get_csc(h, _ptr(d_colptr), _ptr(d_rowind), _ptr(d_cvals), _stream(stream))
     if st != TOMO_OK:
@@ -227,6 +234,13 @@ class TomoLsqr:
         out = torch.empty(self.n if transpose else self.m, dtype=torch.float64, device=x.device)
         tomo_lsqr_spmv(self.h, transpose, x, out)
         return out
+
+    def update_values(self, vals):
+        """New values on the same pattern (CSR order); the tensor replaces the borrowed value array."""
+        assert vals.is_cuda and vals.dtype == self._keep[2].dtype and vals.numel() == self.nnz
+        vals = vals.contiguous()
+        tomo_lsqr_update_values(self.h, vals)
+        self._keep = (self._keep[0], self._keep[1], vals)
 
     def csc(self):
         import torch

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtomolsqr.so")
 SOURCES = ["tomo_lsqr.cu"]
-HEADERS = ["accum.cuh", "state.cuh", "tails.cuh", "kernels.cuh", "wstream.cuh", "compress.cuh", "multi.cuh", "build.cuh", os.path.join("..", "..", "include", "tomo_lsqr.h")]
+HEADERS = ["accum.cuh", "state.cuh", "tails.cuh", "kernels.cuh", "wstream.cuh", "compress.cuh", "wspmm.cuh", "multi.cuh", "build.cuh", os.path.join("..", "..", "include", "tomo_lsqr.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
@@ -39,8 +39,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
-    tune = [f"-D{k}={os.environ[k]}" for k in ("TOMO_CH", "TOMO_W", "TOMO_S", "TOMO_PF") if os.environ.get(k)]  # kernel-shape sweeps
-    cmd = [_nvcc()] + NVCC_FLAGS + tune + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True, cwd=CSRC)
     os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -80,13 +80,21 @@ __global__ void k_tr_count(const int64_t* __restrict__ ptr, const int32_t* __res
   for (int64_t q = s + lane; q < e; q += 32) atomicAdd(my + idx[q], 1u);
 }
 
-// pass B: thread j scans cnt[0..T)[j]; coltotal[j] = column length
+// pass B: thread j scans cnt[0..T)[j] (eight independent loads in flight); coltotal[j] = column length
 __global__ void k_tr_colscan(int T, int64_t n, uint32_t* cnt, int64_t* coltotal) {
   const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   uint32_t run = 0;
-  for (int t = 0; t < T; ++t) {
-    uint32_t c = cnt[(int64_t)t * n + j];
+  int t = 0;
+  for (; t + 8 <= T; t += 8) {
+    uint32_t c[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) c[u] = cnt[(int64_t)(t + u) * n + j];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { cnt[(int64_t)(t + u) * n + j] = run; run += c[u]; }
+  }
+  for (; t < T; ++t) {
+    const uint32_t c = cnt[(int64_t)t * n + j];
     cnt[(int64_t)t * n + j] = run;
     run += c;
   }
@@ -113,11 +121,12 @@ __global__ void __launch_bounds__(1024) k_exscan(const int64_t* __restrict__ in,
   for (int64_t i = b; i < e; ++i) { int64_t v = in[i]; out[i] = acc; acc += v; }
 }
 
-// pass C
-template <typename VT>
+// pass C.  pos (optional): pos[q] = CSC slot of CSR element q, the permutation tomo_lsqr_update_values replays;
+// rowind / cvals may be NULL when only the permutation is wanted.
+template <typename VT, typename PT>
 __global__ void k_tr_scatter(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx,
                              const VT* __restrict__ val, const int32_t* __restrict__ chunk, int T, int64_t n,
-                             uint32_t* cnt, const int64_t* __restrict__ colptr, int32_t* rowind, VT* cvals) {
+                             uint32_t* cnt, const int64_t* __restrict__ colptr, int32_t* rowind, VT* cvals, PT* pos) {
   const int lane = threadIdx.x & 31;
   const int t = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   if (t >= T) return;
@@ -126,15 +135,33 @@ __global__ void k_tr_scatter(const int64_t* __restrict__ ptr, const int32_t* __r
     const int64_t s = ptr[r], e = ptr[r + 1];
     for (int64_t q = s + lane; q < e; q += 32) {
       const int32_t c = idx[q];
-      const VT v = val[q];
       const uint32_t k = __ldcg(my + c);
       __stcg(my + c, k + 1u);
       const int64_t d = colptr[c] + (int64_t)k;
-      rowind[d] = r;
-      cvals[d] = v;
+      if (rowind) { rowind[d] = r; cvals[d] = val[q]; }
+      if (pos) pos[q] = (PT)d;
     }
     __syncwarp();
   }
+}
+
+// NEXT-4 (every outer iteration re-evaluates G on the same rays and solves
+// again): new values in CSR order go to their CSC slots.  Consecutive rows of one station pair hit adjacent slots
+// of the same columns, so the 8-byte scattered writes merge in L2.
+template <typename VT, typename PT>
+__global__ void k_update_values(const VT* __restrict__ val, const PT* __restrict__ pos, int64_t nnz, VT* __restrict__ cvals) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += stride) cvals[pos[q]] = val[q];
+}
+
+// all values finite? (the check create makes, for a refreshed value array)
+template <typename VT>
+__global__ void k_values_finite(const VT* __restrict__ val, int64_t nnz, int* flags) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  int bad = 0;
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < nnz; q += stride)
+    if (!(fabs((double)val[q]) <= 1.79769313486231570815e308)) bad = BAD_VALUE;
+  if (bad) atomicOr(flags, bad);
 }
 
 }  // namespace tomo

@@ -10,11 +10,13 @@
 //
 // Format, per tile of TILE consecutive elements (tiles are aligned to multiples of TILE, like the warp ranges
 // of wstream.cuh), one record at byte offset coff[t] (16-byte aligned):
-//     TILE/8 bytes   flag bits: bit i = "element i continues a run": idx[e] == idx[e-1] + 1 and e % 32 != 0
-//                    (a head is forced at every 32-element step, so a step decodes without looking back)
-//     4 bytes per head: idx[e] of every element whose flag is 0, in element order; padded to 16 bytes.
-// Decoding (k_wstream, FMT 1): head of lane l in a step = highest clear flag at or below l (find-leading-one),
-// its position in the head list = number of clear flags before it (popc), index = head value + distance.
+//     TILE/8 bytes   head bits, one 32-bit word per 32-element step: bit i = "element i starts a run":
+//                    i == 0 (a head is forced at every step, so a step decodes without looking back) or
+//                    idx[e] != idx[e-1] + 1
+//     4 bytes per head: idx[e] - i for every head, in element order (biased by its position i in the step, so
+//                    that the lane adds only its own lane number); padded to 16 bytes.
+// Decoding (k_wstream, FMT 1): r = popc(H & lanes <= mine) counts the heads up to and including mine, the last
+// of them is my run's head: index = heads[heads before this step + r - 1] + lane.  One popc, one shared load.
 // Runs may cross row boundaries: row membership comes from the row pointers, not from the index stream.
 #pragma once
 #include <cuda_runtime.h>
@@ -56,10 +58,9 @@ __global__ void k_cz_fill(const int32_t* __restrict__ idx, int64_t nnz, int64_t 
       bool cont = true;
       int32_t c = 0;
       if (e < nnz) { c = idx[e]; cont = (lane != 0) && (c == idx[e - 1] + 1); }
-      const unsigned F = __ballot_sync(0xffffffffu, cont);
-      const unsigned H = ~F;
-      if (lane == 0) flags[s] = F;
-      if (!cont) heads[hb + __popc(H & ((1u << lane) - 1u))] = c;
+      const unsigned H = __ballot_sync(0xffffffffu, !cont);
+      if (lane == 0) flags[s] = H;
+      if (!cont) heads[hb + __popc(H & ((1u << lane) - 1u))] = c - lane;
       hb += __popc(H);
     }
     // padding words of the record stay unwritten: they are never read (only copied)

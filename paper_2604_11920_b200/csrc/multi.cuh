@@ -1,8 +1,6 @@
-// multi.cuh — the multi-right-hand-side variant (BASELINE configs[3]): eight independent
-// LSQR recurrences that SHARE every pass over A and A^T.  Vectors are row-major blocks (len x 8): one
-// element of the matrix is read once and multiplied with a 64-byte row of the gathered block, so the
-// HBM stream of `idx`/`val` is paid once per iteration for all eight systems; the gather (64 B per
-// nonzero through L1/L2) and, in dd mode, the fp64 pipe become the limits.
+// multi.cuh — the fused vector kernels of the multi-right-hand-side variant (BASELINE
+// configs[3]): eight independent LSQR / LSMR recurrences that SHARE every pass over A and A^T.  Vectors are
+// row-major blocks (len x 8); the two sparse products live in wspmm.cuh.
 //
 // Each right-hand side has its own device-resident Scalars (sc[0..8)), its own stopping tests and stop
 // flag; a stopped side is frozen: its columns are no longer written.  Fewer than eight sides are padded
@@ -11,10 +9,10 @@
 #include "accum.cuh"
 #include "state.cuh"
 #include "tails.cuh"
+#include "wspmm.cuh"
 
 namespace tomo {
 
-constexpr int kR = 8;             // right-hand sides per pass
 constexpr int kMThreads = 256;    // block size of the multi kernels
 constexpr int kMWarps = kMThreads / 32;
 
@@ -54,131 +52,6 @@ __device__ __forceinline__ bool finish_columns(Acc<MODE> blocksum, double2* part
   for (int b = 0; b < (int)gridDim.x; ++b) { Acc<MODE> o; o.unpack(__ldcg(partials + (size_t)b * kR + threadIdx.x)); a.merge(o); }
   total = a.value();
   return true;
-}
-
-// Y[r][k] <- sum_j a_rj X[j][k] (+ c_k * Y[r][k] * sy_k), ||Y[:,k]||^2, for k = 0..7; rows of the CSR-like
-// triple are dealt to the warps of a block round-robin inside the block's static range part[b]..part[b+1].
-template <int MODE, typename VT, int OP>
-__global__ void __launch_bounds__(kMThreads) k_spmm8(const int64_t* __restrict__ ptr, const int32_t* __restrict__ idx,
-                                                     const VT* __restrict__ val, const double* __restrict__ X,
-                                                     double* __restrict__ Y, const int32_t* __restrict__ part, Scalars* sc,
-                                                     double2* partials) {
-  __shared__ double2 s_slots[kMWarps][kR];
-  __shared__ double s_c[kR], s_sx[kR], s_sy[kR];
-  __shared__ int s_skip[kR], s_flag, s_any;
-  if (threadIdx.x < kR) {
-    const Scalars* s = sc + threadIdx.x;
-    const int skip = s->stop || (OP == OP_K2 && s->beta_zero);
-    s_skip[threadIdx.x] = skip;
-    s_c[threadIdx.x] = (OP == OP_K1) ? -s->alpha : (OP == OP_K2 ? -s->beta : 0.0);
-    s_sx[threadIdx.x] = (OP == OP_K2 || OP == OP_K2_INIT) ? s->rbeta : 1.0;
-    s_sy[threadIdx.x] = (OP == OP_K1) ? s->rbeta : 1.0;
-  }
-  if (threadIdx.x == 0) s_any = 0;
-  __syncthreads();
-  if (threadIdx.x < kR && !sc[threadIdx.x].stop) s_any = 1;
-  __syncthreads();
-  if (!s_any) return;  // every side has stopped: nothing changes any more
-  constexpr bool SCALE_X = (OP == OP_K2 || OP == OP_K2_INIT);
-  // Lane layout: lane = 4*es + j.  The warp takes 8 consecutive elements per step (es = 0..7); the four
-  // lanes of an element each gather 16 bytes (sides 2j, 2j+1) of its 64-byte row of X, so one warp load
-  // touches 8 rows = 8 L1 wavefronts for 8 elements (a lane-per-element layout with 64-byte gathers costs
-  // four times as many wavefronts and is bound by them).
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, es = lane >> 2, j = lane & 3;
-  const double sx0 = s_sx[2 * j], sx1 = s_sx[2 * j + 1];
-  const double c0 = s_c[2 * j], c1 = s_c[2 * j + 1], sy0 = s_sy[2 * j], sy1 = s_sy[2 * j + 1];
-  const bool skip0 = s_skip[2 * j] != 0, skip1 = s_skip[2 * j + 1] != 0;
-  Acc<MODE> nsq0, nsq1;
-  nsq0.zero(); nsq1.zero();
-  const int R0 = part[blockIdx.x], R1 = part[blockIdx.x + 1];
-  const double2* X2 = reinterpret_cast<const double2*>(X);
-  for (int r = R0 + warp; r < R1; r += kMWarps) {
-    const int64_t s = ptr[r], e = ptr[r + 1];
-    Acc<MODE> a0, a1;
-    a0.zero(); a1.zero();
-    int64_t q = s + es;
-    for (; q + 56 < e; q += 64) {  // eight steps in flight
-      int32_t cc[8];
-      double vv[8];
-      double2 xx[8];
-#pragma unroll
-      for (int u = 0; u < 8; ++u) { cc[u] = idx[q + 8 * u]; vv[u] = (double)val[q + 8 * u]; }
-#pragma unroll
-      for (int u = 0; u < 8; ++u) xx[u] = __ldg(X2 + (size_t)cc[u] * (kR / 2) + j);
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        if (SCALE_X) { xx[u].x = xx[u].x * sx0; xx[u].y = xx[u].y * sx1; }
-        a0.mac(vv[u], xx[u].x);
-        a1.mac(vv[u], xx[u].y);
-      }
-    }
-    for (; q < e; q += 8) {
-      const int32_t c = idx[q];
-      const double v = (double)val[q];
-      double2 x2 = __ldg(X2 + (size_t)c * (kR / 2) + j);
-      if (SCALE_X) { x2.x = x2.x * sx0; x2.y = x2.y * sx1; }
-      a0.mac(v, x2.x);
-      a1.mac(v, x2.y);
-    }
-    // sum over the eight element slots (lane bits 2..4), same order in both partners
-#pragma unroll
-    for (int off = 16; off >= 4; off >>= 1) {
-      Acc<MODE> o0, o1;
-      double2 p0 = a0.pack(), p1 = a1.pack();
-      p0.x = __shfl_xor_sync(0xffffffffu, p0.x, off); p0.y = __shfl_xor_sync(0xffffffffu, p0.y, off);
-      p1.x = __shfl_xor_sync(0xffffffffu, p1.x, off); p1.y = __shfl_xor_sync(0xffffffffu, p1.y, off);
-      o0.unpack(p0); o1.unpack(p1);
-      if (lane & off) { o0.merge(a0); a0 = o0; o1.merge(a1); a1 = o1; } else { a0.merge(o0); a1.merge(o1); }
-    }
-    if (lane < 4) {  // lane j: sides 2j and 2j+1 of this row
-      double2* yp = reinterpret_cast<double2*>(Y + (size_t)r * kR) + j;
-      double2 yo = make_double2(0.0, 0.0);
-      if (OP == OP_K1 || OP == OP_K2) yo = *yp;
-      double yn0, yn1;
-      if (OP == OP_K1 || OP == OP_K2) {
-        double y0 = yo.x, y1 = yo.y;
-        if (OP == OP_K1) { y0 = y0 * sy0; y1 = y1 * sy1; }
-        if (MODE == 0) { yn0 = fma(c0, y0, a0.value()); yn1 = fma(c1, y1, a1.value()); }
-        else { a0.mac(c0, y0); yn0 = a0.value(); a1.mac(c1, y1); yn1 = a1.value(); }
-      } else {
-        yn0 = a0.value(); yn1 = a1.value();
-      }
-      if (OP == OP_K1 || OP == OP_K2) {  // a stopped side keeps its old column
-        if (skip0) yn0 = yo.x;
-        if (skip1) yn1 = yo.y;
-        *yp = make_double2(yn0, yn1);
-      } else if (!(skip0 && skip1)) {
-        double2 old = (skip0 || skip1) ? *yp : make_double2(0.0, 0.0);
-        *yp = make_double2(skip0 ? old.x : yn0, skip1 ? old.y : yn1);
-      }
-      if (OP != OP_PLAIN) {
-        if (!skip0) nsq0.mac(yn0, yn0);
-        if (!skip1) nsq1.mac(yn1, yn1);
-      }
-    }
-  }
-  // lanes 0..3 hold the sums of sides (2j, 2j+1): spread them to lanes 0..7 as side = lane
-  Acc<MODE> nsq;
-  {
-    const int src = (lane & 7) >> 1;
-    double2 p0 = nsq0.pack(), p1 = nsq1.pack();
-    p0.x = __shfl_sync(0xffffffffu, p0.x, src); p0.y = __shfl_sync(0xffffffffu, p0.y, src);
-    p1.x = __shfl_sync(0xffffffffu, p1.x, src); p1.y = __shfl_sync(0xffffffffu, p1.y, src);
-    nsq.unpack((lane & 1) ? p1 : p0);
-  }
-  if (OP == OP_PLAIN) return;
-  Acc<MODE> bs = block_columns<MODE>(nsq, s_slots);
-  double total = 0.0;
-  if (finish_columns<MODE>(bs, partials, &sc->ticket[0], &s_flag, total)) {
-    Scalars* s = sc + threadIdx.x;
-    if (!s->stop) {
-      const bool skipped = (OP == OP_K2 && s->beta_zero);
-      if (OP == OP_K1) tail_k1(s, total);
-      if (OP == OP_K2) tail_k2(s, skipped ? 0.0 : total);
-      if (OP == OP_K2_INIT) tail_init_v(s, total);
-    }
-    if (threadIdx.x == 0) sc->ticket[0] = 0u;
-  }
 }
 
 // Fused vector kernels on len x 8 blocks; element e = i*8 + k belongs to side k = e & 7, which is fixed per

@@ -81,7 +81,7 @@ struct tomo_lsqr_s {
   int solver = 0;  // 0 LSQR, 1 LSMR (set per solve)
   // shared-pass multi-RHS state (multi.cuh): len x 8 blocks, eight Scalars, static row partitions
   double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr, *mH = nullptr; Scalars* msc = nullptr; Scalars* h_msc = nullptr;
-  int32_t *mpart_r = nullptr, *mpart_c = nullptr; double2* mpartials = nullptr; int MG = 0, multi_shared = 1;
+  CtaRec8* cta_rec8 = nullptr; double2* mpartials = nullptr; int MG = 0, multi_shared = 1;
   bool multi_ready = false;              // every m* allocation succeeded and the partitions were computed
   PollWord* h_mpoll = nullptr;           // pinned: two slots of eight {itn, istop, stop} words
   cudaGraphExec_t mgexec = nullptr; int mgraph_k = 0, mgraph_mode = -1;
@@ -93,9 +93,10 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 96, pdl = 1, compress = 0;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 320, pdl = 1, compress = 0;
   // info
-  int sms = 0; double create_ms = 0, transpose_ms = 0, scratch_bytes = 0;
+  int sms = 0; double create_ms = 0, transpose_ms = 0, transpose_kernels_ms = 0, update_ms = 0, scratch_bytes = 0;
+  void* pos = nullptr; bool pos_wide = false;   // CSR element -> CSC slot (built by the first tomo_lsqr_update_values)
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
   double kernels_enqueued = 0;  // cumulative count of this library's kernel launches (graph nodes included)
   std::vector<cudaEvent_t> prof_ev;
@@ -309,12 +310,20 @@ tomo_status_t build_compressed(tomo_lsqr_s* h, int d, cudaStream_t st) {
 // ------------------------------------------------------------------------------------------------
 namespace {
 
+// The transpose passes (build.cuh).  only_pos = false: allocate and fill the CSC copy (create).  only_pos = true:
+// the CSC copy exists; replay the passes to record the permutation pos[q] = CSC slot of CSR element q
+// (uint32 when nnz < 2^32, else int64) that tomo_lsqr_update_values needs; built on its first call.
 template <typename VT>
-tomo_status_t build_csc(tomo_lsqr_s* h, cudaStream_t st) {
+tomo_status_t build_csc(tomo_lsqr_s* h, cudaStream_t st, bool only_pos) {
   const int64_t m = h->m, n = h->n, nnz = h->nnz;
-  CK(cudaMalloc(&h->colptr, sizeof(int64_t) * (n + 1)));
-  CK(cudaMalloc(&h->rowind, sizeof(int32_t) * std::max<int64_t>(nnz, 1)));
-  CK(cudaMalloc(&h->cvals, sizeof(VT) * std::max<int64_t>(nnz, 1)));
+  if (!only_pos) {
+    CK(cudaMalloc(&h->colptr, sizeof(int64_t) * (n + 1)));
+    CK(cudaMalloc(&h->rowind, sizeof(int32_t) * std::max<int64_t>(nnz, 1)));
+    CK(cudaMalloc(&h->cvals, sizeof(VT) * std::max<int64_t>(nnz, 1)));
+  } else {
+    h->pos_wide = nnz >= ((int64_t)1 << 32);
+    CK(cudaMalloc(&h->pos, (h->pos_wide ? sizeof(int64_t) : sizeof(uint32_t)) * std::max<int64_t>(nnz, 1)));
+  }
   // number of row chunks (= warps): bounded by the scratch budget T*n*4 bytes <= 4 GB
   int64_t T = std::min<int64_t>((int64_t)h->sms * 16, std::max<int64_t>(32, (int64_t)(4.0e9 / (4.0 * (double)n))));
   T = std::max<int64_t>(1, std::min<int64_t>(T, m));
@@ -326,22 +335,39 @@ tomo_status_t build_csc(tomo_lsqr_s* h, cudaStream_t st) {
   if (e != cudaSuccess) { cudaFree(chunk); cudaFree(cnt); return cuda_fail(e, "cudaMalloc(coltotal)"); }
   h->scratch_bytes = (double)(sizeof(uint32_t) * T * n + sizeof(int64_t) * n + sizeof(int32_t) * (T + 1));
   tomo_status_t rc = TOMO_OK;
+  cudaEvent_t k0 = nullptr, k1 = nullptr;
+  cudaEventCreate(&k0); cudaEventCreate(&k1);
   do {
     const int tb = 128;
+    cudaEventRecord(k0, st);
     k_partition<<<(int)((T + 1 + tb - 1) / tb), tb, 0, st>>>(h->rowptr, m, (int)T, 1, 1, chunk);
     k_partition_fix<<<1, 32, 0, st>>>((int)T, chunk);
     if ((e = cudaMemsetAsync(cnt, 0, sizeof(uint32_t) * T * n, st)) != cudaSuccess) break;
     const int wb = (int)((T + kWarps - 1) / kWarps);
     k_tr_count<<<wb, kThreads, 0, st>>>(h->rowptr, h->colind, chunk, (int)T, n, cnt);
     k_tr_colscan<<<(int)((n + 255) / 256), 256, 0, st>>>((int)T, n, cnt, coltotal);
-    k_exscan<<<1, 1024, 0, st>>>(coltotal, n, h->colptr);
-    k_tr_scatter<VT><<<wb, kThreads, 0, st>>>(h->rowptr, h->colind, (const VT*)h->vals, chunk, (int)T, n, cnt,
-                                             h->colptr, h->rowind, (VT*)h->cvals);
+    if (!only_pos) {
+      k_exscan<<<1, 1024, 0, st>>>(coltotal, n, h->colptr);
+      k_tr_scatter<VT, uint32_t><<<wb, kThreads, 0, st>>>(h->rowptr, h->colind, (const VT*)h->vals, chunk, (int)T, n, cnt,
+                                                         h->colptr, h->rowind, (VT*)h->cvals, (uint32_t*)nullptr);
+    } else if (h->pos_wide) {
+      k_tr_scatter<VT, int64_t><<<wb, kThreads, 0, st>>>(h->rowptr, h->colind, (const VT*)h->vals, chunk, (int)T, n, cnt,
+                                                        h->colptr, (int32_t*)nullptr, (VT*)nullptr, (int64_t*)h->pos);
+    } else {
+      k_tr_scatter<VT, uint32_t><<<wb, kThreads, 0, st>>>(h->rowptr, h->colind, (const VT*)h->vals, chunk, (int)T, n, cnt,
+                                                         h->colptr, (int32_t*)nullptr, (VT*)nullptr, (uint32_t*)h->pos);
+    }
+    cudaEventRecord(k1, st);
     if ((e = cudaGetLastError()) != cudaSuccess) break;
     e = cudaStreamSynchronize(st);
+    float ms = 0;
+    if (e == cudaSuccess && !only_pos && cudaEventElapsedTime(&ms, k0, k1) == cudaSuccess) h->transpose_kernels_ms = ms;
   } while (0);
+  if (k0) cudaEventDestroy(k0);
+  if (k1) cudaEventDestroy(k1);
   if (e != cudaSuccess) rc = cuda_fail(e, "CSR->CSC transpose");
   cudaFree(chunk); cudaFree(cnt); cudaFree(coltotal);
+  if (rc != TOMO_OK && only_pos) { cudaFree(h->pos); h->pos = nullptr; }
   return rc;
 }
 
@@ -351,8 +377,8 @@ void free_handle(tomo_lsqr_s* h) {
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   for (int i = 0; i < 2; ++i) if (h->ev_poll[i]) cudaEventDestroy(h->ev_poll[i]);
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
-  cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals);
-  cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->mH); cudaFree(h->msc); cudaFree(h->mpart_r); cudaFree(h->mpart_c);
+  cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals); cudaFree(h->pos);
+  cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->mH); cudaFree(h->msc); cudaFree(h->cta_rec8);
   cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->h_mpoll) cudaFreeHost(h->h_mpoll); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   cudaFree(h->cta_rec);
@@ -411,7 +437,7 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
     if (flags) { rc = TOMO_ERR_BAD_CSR; break; }
     // --- transpose ---
     cudaEventRecord(e1, st);
-    rc = (vt == TOMO_VAL_F64) ? build_csc<double>(h, st) : build_csc<float>(h, st);
+    rc = (vt == TOMO_VAL_F64) ? build_csc<double>(h, st, false) : build_csc<float>(h, st, false);
     if (rc != TOMO_OK) break;
     cudaEventRecord(e2, st);
     // --- work space ---
@@ -677,20 +703,47 @@ __global__ void k_col_scatter(const double* __restrict__ in, int nrhs, int r, in
 
 namespace {
 
+// block products (wspmm.cuh): same split points as the single-side kernel of the direction, a 2-stage ring per warp
+// (96 KB of shared memory: the rest of the SM's 228 KB is L1 for the 64-byte gathers)
+using WM = WCfg<TOMO_TILE, 2, TOMO_W>;
+
+template <int MODE, typename VT, int OP>
+void launch_spmm_t(const tomo_lsqr_s* h, bool transpose, const double* X, double* Y, cudaStream_t st) {
+  const Dir& d = h->dir[transpose ? 1 : 0];
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)h->SG); cfg.blockDim = dim3(WM::THREADS);
+  cfg.dynamicSmemBytes = MSmem<WM, VT>::kTotal; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = h->pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, k_wspmm8<WM, MODE, VT, OP>, d.ptr, (const int32_t*)d.rid, d.idx, (const VT*)d.val, h->nnz, d.nrows,
+                     (const int32_t*)d.erows, d.n_empty, X, Y, (const int64_t*)d.wE, (const int32_t*)d.wR, h->cta_rec8, h->msc,
+                     h->mpartials);
+}
+
 template <int OP>
 void launch_spmm(const tomo_lsqr_s* h, bool transpose, const double* X, double* Y, cudaStream_t st) {
-  const int64_t* ptr = transpose ? h->colptr : h->rowptr;
-  const int32_t* idx = transpose ? h->rowind : h->colind;
-  const int32_t* part = transpose ? h->mpart_c : h->mpart_r;
   if (h->vt == TOMO_VAL_F64) {
-    const double* val = (const double*)(transpose ? h->cvals : h->vals);
-    if (h->accumulate) k_spmm8<1, double, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
-    else k_spmm8<0, double, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+    if (h->accumulate) launch_spmm_t<1, double, OP>(h, transpose, X, Y, st); else launch_spmm_t<0, double, OP>(h, transpose, X, Y, st);
   } else {
-    const float* val = (const float*)(transpose ? h->cvals : h->vals);
-    if (h->accumulate) k_spmm8<1, float, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
-    else k_spmm8<0, float, OP><<<h->MG, kMThreads, 0, st>>>(ptr, idx, val, X, Y, part, h->msc, h->mpartials);
+    if (h->accumulate) launch_spmm_t<1, float, OP>(h, transpose, X, Y, st); else launch_spmm_t<0, float, OP>(h, transpose, X, Y, st);
   }
+}
+
+template <int MODE, typename VT>
+cudaError_t spmm_attr_ops() {
+  cudaError_t e;
+  const int smem = (int)MSmem<WM, VT>::kTotal;
+  if ((e = cudaFuncSetAttribute(k_wspmm8<WM, MODE, VT, OP_K1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_wspmm8<WM, MODE, VT, OP_K2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_wspmm8<WM, MODE, VT, OP_K2_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+}
+cudaError_t set_multi_attributes(tomo_valtype_t vt) {
+  cudaError_t e;
+  if (vt == TOMO_VAL_F64) { if ((e = spmm_attr_ops<0, double>()) != cudaSuccess) return e; return spmm_attr_ops<1, double>(); }
+  if ((e = spmm_attr_ops<0, float>()) != cudaSuccess) return e;
+  return spmm_attr_ops<1, float>();
 }
 
 template <int VOP>
@@ -717,7 +770,7 @@ tomo_status_t ensure_multi(tomo_lsqr_s* h, cudaStream_t st) {
   const int MG = h->sms * 8;
   double *mU = nullptr, *mV = nullptr, *mW = nullptr, *mX = nullptr, *mH = nullptr;
   Scalars *msc = nullptr, *h_msc = nullptr; PollWord* h_mpoll = nullptr;
-  int32_t *pr = nullptr, *pc = nullptr; double2* mp = nullptr;
+  CtaRec8* cr = nullptr; double2* mp = nullptr;
   cudaError_t e = cudaSuccess;
   do {
     if ((e = cudaMalloc(&mU, sizeof(double) * m * kR)) != cudaSuccess) break;
@@ -728,25 +781,18 @@ tomo_status_t ensure_multi(tomo_lsqr_s* h, cudaStream_t st) {
     if ((e = cudaMalloc(&msc, sizeof(Scalars) * kR)) != cudaSuccess) break;
     if ((e = cudaMallocHost(&h_msc, sizeof(Scalars) * kR)) != cudaSuccess) break;
     if ((e = cudaMallocHost(&h_mpoll, sizeof(PollWord) * kR * 2)) != cudaSuccess) break;
-    if ((e = cudaMalloc(&pr, sizeof(int32_t) * (MG + 1))) != cudaSuccess) break;
-    if ((e = cudaMalloc(&pc, sizeof(int32_t) * (MG + 1))) != cudaSuccess) break;
+    if ((e = cudaMalloc(&cr, sizeof(CtaRec8) * h->sms)) != cudaSuccess) break;
     if ((e = cudaMalloc(&mp, sizeof(double2) * kR * MG)) != cudaSuccess) break;
-    const int tb = 128, gb = (MG + 1 + tb - 1) / tb;
-    k_partition<<<gb, tb, 0, st>>>(h->rowptr, m, MG, 16, 1, pr);
-    k_partition_fix<<<1, 32, 0, st>>>(MG, pr);
-    k_partition<<<gb, tb, 0, st>>>(h->colptr, n, MG, 16, 1, pc);
-    k_partition_fix<<<1, 32, 0, st>>>(MG, pc);
-    if ((e = cudaGetLastError()) != cudaSuccess) break;
-    e = cudaStreamSynchronize(st);
+    e = set_multi_attributes(h->vt);
   } while (0);
   if (e != cudaSuccess) {
-    cudaFree(mU); cudaFree(mV); cudaFree(mW); cudaFree(mX); cudaFree(mH); cudaFree(msc); cudaFree(pr); cudaFree(pc); cudaFree(mp);
+    cudaFree(mU); cudaFree(mV); cudaFree(mW); cudaFree(mX); cudaFree(mH); cudaFree(msc); cudaFree(cr); cudaFree(mp);
     if (h_msc) cudaFreeHost(h_msc);
     if (h_mpoll) cudaFreeHost(h_mpoll);
     return cuda_fail(e, "block-solve work space");
   }
   h->mU = mU; h->mV = mV; h->mW = mW; h->mX = mX; h->mH = mH; h->msc = msc; h->h_msc = h_msc; h->h_mpoll = h_mpoll;
-  h->mpart_r = pr; h->mpart_c = pc; h->mpartials = mp; h->MG = MG;
+  h->cta_rec8 = cr; h->mpartials = mp; h->MG = MG;
   h->multi_ready = true;
   return TOMO_OK;
 }
@@ -757,6 +803,7 @@ tomo_status_t solve_multi_shared(tomo_lsqr_s* h, int solver, int32_t nrhs, const
                                  int32_t max_iters, double* d_X, tomo_lsqr_result_t* res, cudaStream_t st) {
   const int64_t m = h->m, n = h->n;
   { tomo_status_t rc = ensure_multi(h, st); if (rc != TOMO_OK) return rc; }
+  { tomo_status_t rc = rebuild_partitions(h, st); if (rc != TOMO_OK) return rc; }
   h->solver = solver;
   const int k = h->check_every;
   const int gkey = h->accumulate + 2 * solver;
@@ -892,6 +939,49 @@ extern "C" tomo_status_t tomo_lsmr_solve_multi(tomo_lsqr_t h, int32_t nrhs, cons
   return solve_multi_any(h, 1, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, (cudaStream_t)cuda_stream);
 }
 
+namespace {
+template <typename VT>
+tomo_status_t update_values_t(tomo_lsqr_s* h, const VT* d_vals, cudaStream_t st) {
+  int* d_flag = nullptr;
+  CK(cudaMalloc(&d_flag, sizeof(int)));
+  cudaMemsetAsync(d_flag, 0, sizeof(int), st);
+  k_values_finite<VT><<<h->sms * 8, 256, 0, st>>>(d_vals, h->nnz, d_flag);
+  int flag = 0;
+  cudaError_t e = cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_flag);
+  if (e != cudaSuccess) return cuda_fail(e, "value check");
+  if (flag) return TOMO_ERR_BAD_CSR;  // nothing has been touched yet
+  if (!h->pos && h->nnz > 0) { tomo_status_t rc = build_csc<VT>(h, st, true); if (rc != TOMO_OK) return rc; }
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  cudaEventRecord(e0, st);
+  if (h->nnz > 0) {
+    if (h->pos_wide) k_update_values<VT, int64_t><<<h->sms * 16, 256, 0, st>>>(d_vals, (const int64_t*)h->pos, h->nnz, (VT*)h->cvals);
+    else k_update_values<VT, uint32_t><<<h->sms * 16, 256, 0, st>>>(d_vals, (const uint32_t*)h->pos, h->nnz, (VT*)h->cvals);
+  }
+  cudaEventRecord(e1, st);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  float ms = 0;
+  if (e == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess) h->update_ms = ms;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  if (e != cudaSuccess) return cuda_fail(e, "value refresh");
+  h->vals = d_vals;
+  h->dir[0].val = d_vals;
+  return TOMO_OK;
+}
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_update_values(tomo_lsqr_t h, const void* d_vals, void* cuda_stream) {
+  if (!h || (h->nnz > 0 && !d_vals)) return TOMO_ERR_INVALID_ARG;
+  { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
+  if (h->nnz > 0 && !is_device_ptr(d_vals)) return TOMO_ERR_NOT_DEVICE_PTR;
+  if ((uintptr_t)d_vals & 15u) return TOMO_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  return h->vt == TOMO_VAL_F64 ? update_values_t<double>(h, (const double*)d_vals, st) : update_values_t<float>(h, (const float*)d_vals, st);
+}
+
 extern "C" tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const double* d_in, double* d_out, void* cuda_stream) {
   if (!h || !d_in || !d_out || (transpose != 0 && transpose != 1)) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_in) || !is_device_ptr(d_out)) return TOMO_ERR_NOT_DEVICE_PTR;
@@ -945,6 +1035,8 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   const double vb = h->vt == TOMO_VAL_F64 ? 8.0 : 4.0;
   if (k == "create_ms") *out = h->create_ms;
   else if (k == "transpose_ms") *out = h->transpose_ms;
+  else if (k == "transpose_kernels_ms") *out = h->transpose_kernels_ms;
+  else if (k == "update_ms") *out = h->update_ms;
   else if (k == "csc_bytes") *out = (double)h->nnz * (4.0 + vb) + 8.0 * (double)(h->n + 1);
   else if (k == "scratch_bytes") *out = h->scratch_bytes;
   else if (k == "compress_bytes_rows") *out = (double)h->dir[0].cbytes + 8.0 * (double)((h->nnz + WC::TILE - 1) / WC::TILE + 1);

@@ -264,15 +264,15 @@ __device__ __forceinline__ int win_load(const WCtx& cx, int rbase) {
   return p >= (int64_t)kBig ? kBig : (int)p;
 }
 // start of row r (uniform), wbase <= r < wbase + 64
-template <int MODE>
-__device__ __forceinline__ int win_get(const WSweep<MODE>& st, int r) {
+template <typename ST>
+__device__ __forceinline__ int win_get(const ST& st, int r) {
   const int i = r - st.wbase;
   const int a = __shfl_sync(0xffffffffu, st.S, i & 31), b = __shfl_sync(0xffffffffu, st.S2, i & 31);
   return i < 32 ? a : b;
 }
 // keep cur + 1 inside the first half of the window
-template <int MODE>
-__device__ __forceinline__ void win_advance(WSweep<MODE>& st, const WCtx& cx) {
+template <typename ST>
+__device__ __forceinline__ void win_advance(ST& st, const WCtx& cx) {
   while (st.cur + 1 - st.wbase >= 32) {
     st.S = st.S2;
     st.wbase += 32;
@@ -590,19 +590,17 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
 #pragma unroll
         for (int u = 0; u < 8; ++u) cc[u] = si[32 * u];
       } else {
-        // run-compressed index: flag bit = "this element continues the run of the previous one"; a head at
-        // every step start.  index = head[#heads before mine in the tile] + distance to my head
-        const uint32_t* fl = reinterpret_cast<const uint32_t*>(sb);
-        const int32_t* heads = reinterpret_cast<const int32_t*>(sb + TILE / 8);
+        // run-compressed index (compress.cuh): H = head bits of the step; my run's head is the last head at or
+        // below my lane: index = heads[heads before the step + popc(H & lanes <= mine) - 1] + lane
+        const uint32_t* hw = reinterpret_cast<const uint32_t*>(sb) + rr * 8;
+        const int32_t* heads = reinterpret_cast<const int32_t*>(sb + TILE / 8) - 1;
+        const uint32_t le = 0xffffffffu >> (31 - lane);
         int hb = 0;  // heads in the earlier steps of the tile
-        for (int q = 0; q < rr * 8; ++q) hb += 32 - __popc(fl[q]);
+        for (int q = 0; q < rr * 8; ++q) hb += __popc(hw[q - rr * 8]);
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-          const uint32_t H = ~fl[rr * 8 + u];
-          const uint32_t below = (H | 1u) & (0xffffffffu >> (31 - lane));  // lane 0 of a step is always a head
-          const int hpos = 31 - __clz((int)below);
-          const int rank = __popc(H & ((1u << hpos) - 1u));
-          cc[u] = (uint32_t)(heads[hb + rank] + (lane - hpos));
+          const uint32_t H = hw[u];
+          cc[u] = (uint32_t)(heads[hb + __popc(H & le)] + lane);
           hb += __popc(H);
         }
       }

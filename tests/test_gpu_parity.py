@@ -389,6 +389,83 @@ def test_compressed_index_bitwise_equal(tl, g0, cfg0, big):
         assert g.S.info("compress_bytes_rows") < 1.0 * g.S.nnz and g.S.info("compress_bytes_cols") < 2.0 * g.S.nnz
 
 
+# ------------------------------------------------------------------------------- NEXT-4: value refresh -----
+def test_update_values_equals_create_from_scratch(tl, cfg0):
+    """tomo_lsqr_update_values: new values on the same pattern (the outer Gauss-Newton loop of the inversion,
+    PAPER.md P:77/P:81).  update -> solve must equal create-from-scratch -> solve BITWISE, the CSC copy must be the
+    stable transpose of the new matrix, and config 0 must still match the oracle; in-place refresh, a second
+    refresh, the compressed index and the fp32 path included; a NaN is refused and leaves the handle intact."""
+    rng = np.random.default_rng(21)
+    m, n, rp, ci, va = cfg0["m"], cfg0["n"], cfg0["rp"], cfg0["ci"], cfg0["va"]
+    b, damp = cfg0["b"], cfg0["damp"]
+    S = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va))
+    va2 = va * (1.0 + 0.2 * rng.standard_normal(len(va)))
+    S.update_values(dev(va2))
+    cp, ri, cv = (t.cpu().numpy() for t in S.csc())
+    ocp, ori, ocv = oracle.csr_to_csc(m, n, rp, ci, va2)
+    assert np.array_equal(cp, ocp) and np.array_equal(ri, ori) and np.array_equal(cv, ocv)
+    fresh = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va2))
+    for acc in (1, 0):
+        for cz in (0, 1):
+            S.set(accumulate=acc, compress=cz)
+            fresh.set(accumulate=acc, compress=cz)
+            x, res = S.solve(dev(b), damp, 0.0, 0.0, 50)
+            xf, _ = fresh.solve(dev(b), damp, 0.0, 0.0, 50)
+            assert torch.equal(x, xf)
+        o = oracle.lsqr(m, n, rp, ci, va2, b, damp=damp, max_iters=50, mode=acc)
+        assert rel(x.cpu().numpy(), o.x) <= TOL_X50 and res.itn == 50
+        if acc == 1:
+            assert np.array_equal(x.cpu().numpy(), o.x)
+    # refresh in place (the caller overwrites its own array), twice
+    S.set(accumulate=1, compress=0)
+    vals = S._keep[2]
+    va3 = va2 + 0.01 * rng.standard_normal(len(va))
+    vals.copy_(dev(va3))
+    S.update_values(vals)
+    x3, _ = S.solve(dev(b), damp, 0.0, 0.0, 20)
+    o3 = oracle.lsqr(m, n, rp, ci, va3, b, damp=damp, max_iters=20, mode=oracle.DD)
+    assert np.array_equal(x3.cpu().numpy(), o3.x) and S.info("update_ms") > 0
+    # a non-finite value is refused before anything is touched
+    bad = va3.copy(); bad[11] = np.inf
+    with pytest.raises(tl.TomoError) as ei:
+        S.update_values(dev(bad))
+    assert ei.value.status == tl.TOMO_ERR_BAD_CSR
+    assert torch.equal(S.solve(dev(b), damp, 0.0, 0.0, 20)[0], x3)
+    # fp32 storage
+    v32 = va.astype(np.float32)
+    S32 = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(v32))
+    v32b = (va2).astype(np.float32)
+    S32.update_values(dev(v32b))
+    F32 = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(v32b))
+    assert torch.equal(S32.solve(dev(b), damp, 0.0, 0.0, 30)[0], F32.solve(dev(b), damp, 0.0, 0.0, 30)[0])
+
+
+def test_update_values_full_size(big):
+    """The same at config-1 size on a structure with empty-free long rows: x_20 after a refresh is bitwise the x_20
+    of a fresh handle; the refresh pass is timed next to a K1 launch (reported by bench.py)."""
+    s, g = big[1]
+    rng = np.random.default_rng(22)
+    vals = g.S._keep[2]
+    orig = vals.clone()
+    scale = torch.from_numpy(1.0 + 0.1 * rng.standard_normal(8191)).cuda()
+    new = orig * scale.repeat((orig.numel() + 8190) // 8191)[: orig.numel()]
+    g.S.set(accumulate=1, compress=0)
+    g.S.update_values(new)
+    bb = dev(s.rhs(0))
+    x1, _ = g.S.solve(bb, s.damp, 0.0, 0.0, 20)
+    import paper_2604_11920_b200 as tl
+    F = tl.TomoLsqr(s.dims.m, s.dims.n, g.S._keep[0], g.S._keep[1], new)
+    F.set(accumulate=1)
+    xf, _ = F.solve(bb, s.damp, 0.0, 0.0, 20)
+    F.close()
+    assert torch.equal(x1, xf)
+    g.S.update_values(orig)  # back to the generated values for the tests that follow
+    g.S.set(accumulate=0)
+    y = g.S.spmv(dev(np.ones(s.dims.n)))
+    g.S.set(accumulate=1)
+    assert abs(float(y[: s.dims.m_data].sum()) - float(np.repeat(s.ray_lengths(), s.dims.nper).sum())) <= 1e-6 * float(y.abs().sum())
+
+
 def test_fast_mode_reported_next_to_oracle_order_spread(big):
     """P4 (reported, gated only loosely): fast mode vs the plain oracle at full size.  At k = 10 both are
     within rounding; at k = 50 the plain iterate itself moves by ~1e-3 under a change of summation
