@@ -612,10 +612,8 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
         for (int u = 0; u < 8; ++u) xx[u] = (pos0 + 32 * u + lane < cx.len) ? __ldg(x + cc[u]) : 0.0;
       }
     };
-    double xc[8], xn[8];
-    gather(0, xc);
-#pragma unroll 1
-    for (int r = 0; r < nr; ++r) {
+    // round r with its gathers in xc; the gathers of round r + 1 go to xn meanwhile
+    auto body = [&](int r, double (&xc)[8], double (&xn)[8]) {
       if (r + 1 < nr) gather(r + 1, xn);
       const int t = r / RPT, rr = r % RPT;
       const VT* sv = reinterpret_cast<const VT*>(stage_ptr(t % NS) + SM::kIdx) + rr * 256 + lane;
@@ -630,8 +628,15 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
       }
       if (rr == RPT - 1 && t + NS < ntiles) issue_tile(t + NS, true);  // the tile is in registers: its stage is refilled
       consume_round<MODE, OP, SCALE_X>(st, cx, vv, xc, pos0, sx);
+    };
+    double xa[8], xb[8];
+    gather(0, xa);
+#pragma unroll 1
+    for (int r = 0; r < nr; ++r) {  // ONE copy of the round in the code: unrolling twice to swap the gather register sets, or moving
+                                    // the general shape out of line, measured slower (instruction cache / call overhead)
+      body(r, xa, xb);
 #pragma unroll
-      for (int u = 0; u < 8; ++u) xc[u] = xn[u];
+      for (int u = 0; u < 8; ++u) xa[u] = xb[u];
     }
     rec.head = st.h_val; rec.head_state = st.h_state;
   }

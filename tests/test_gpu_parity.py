@@ -644,6 +644,77 @@ def test_edge_cases(tl, g0, cfg0):
     assert res.istop == 0 and not x.any()
 
 
+def test_guard_bands_and_full_overwrite(tl, g0, cfg0):
+    """compute-sanitizer is closed on this pool (gpurun refuses it), so the checks it would make on caller buffers
+    are made by hand: every output array sits between guard bands of a NaN pattern that must stay intact, is
+    pre-filled with NaN and must come back fully overwritten; inputs are followed by NaN bands so that an
+    out-of-range READ would poison the result (which is compared with the oracle)."""
+    pat = float(np.frombuffer(np.uint64(0x7ff8dead0000beef).tobytes(), dtype=np.float64)[0])
+    G = 512
+
+    def banded(n_or_arr):
+        if isinstance(n_or_arr, int):
+            n, src = n_or_arr, None
+        else:
+            n, src = len(n_or_arr), n_or_arr
+        buf = torch.full((n + 2 * G,), pat, dtype=torch.float64, device="cuda")
+        view = buf[G:G + n]
+        if src is not None:
+            view.copy_(torch.from_numpy(np.ascontiguousarray(src)))
+        return buf, view
+
+    def intact(buf, n):
+        raw = buf.view(torch.int64)
+        want = int(np.uint64(0x7ff8dead0000beef).astype(np.int64))
+        return bool((raw[:G] == want).all()) and bool((raw[G + n:] == want).all())
+
+    m, n = g0.m, g0.n
+    rng = np.random.default_rng(3)
+    xv, uv = rng.standard_normal(n), rng.standard_normal(m)
+    for acc in (0, 1):
+        for cz in (0, 1):
+            g0.S.set(accumulate=acc, compress=cz)
+            xin_b, xin = banded(xv)
+            yb, y = banded(m)
+            tl.tomo_lsqr_spmv(g0.S.h, 0, xin, y)
+            assert intact(yb, m) and intact(xin_b, n) and not torch.isnan(y).any()
+            uin_b, uin = banded(uv)
+            ytb, yt = banded(n)
+            tl.tomo_lsqr_spmv(g0.S.h, 1, uin, yt)
+            assert intact(ytb, n) and intact(uin_b, m) and not torch.isnan(yt).any()
+            assert rel(y.cpu().numpy(), oracle.spmv(m, n, g0.rp, g0.ci, g0.va, xv, acc)) <= TOL_SPMV
+            assert rel(yt.cpu().numpy(), oracle.spmv_t(m, n, g0.rp, g0.ci, g0.va, uv, acc)) <= TOL_SPMV
+            bb, b = banded(cfg0["b"])
+            xb, x = banded(n)
+            res = tl.tomo_lsqr_solve(g0.S.h, b, cfg0["damp"], 0.0, 0.0, 20, x)
+            assert res.itn == 20 and intact(xb, n) and intact(bb, m) and not torch.isnan(x).any()
+            res = tl.tomo_lsmr_solve(g0.S.h, b, cfg0["damp"], 0.0, 0.0, 20, x)
+            assert res.itn == 20 and intact(xb, n) and not torch.isnan(x).any()
+    g0.S.set(accumulate=1, compress=0)
+    B = np.stack([cfg0["b"], 0.5 * cfg0["b"], -cfg0["b"]], axis=1)
+    Bb, Bv = banded(B.reshape(-1))
+    Xb, Xv = banded(3 * n)
+    for fn in (tl.tomo_lsqr_solve_multi, tl.tomo_lsmr_solve_multi):
+        Xv.fill_(float("nan"))
+        res = fn(g0.S.h, 3, Bv, cfg0["damp"], 0.0, 0.0, 15, Xv)
+        assert res[0].itn == 15 and intact(Xb, 3 * n) and intact(Bb, 3 * m) and not torch.isnan(Xv).any()
+    # a CSR whose arrays are followed by poison: the last tile of the stream is ragged (nnz % 256 != 0, nnz % 4 != 0)
+    lens = rng.integers(0, 50, size=777)
+    lens[-1] += (3 - int(lens.sum()) % 4) % 4 + 0
+    rp, ci, va = tomogen.random_csr(len(lens), 4000, lens, seed=41)
+    nnz = len(ci)
+    cib = torch.full((nnz + 1024,), 0x7fffffff, dtype=torch.int32, device="cuda")
+    cib[:nnz].copy_(torch.from_numpy(ci))
+    vab, vav = banded(va)
+    S = tl.TomoLsqr(len(lens), 4000, dev(rp), cib[:nnz], vav)
+    xv2 = rng.standard_normal(4000)
+    for acc in (0, 1):
+        S.set(accumulate=acc)
+        y2 = S.spmv(dev(xv2)).cpu().numpy()
+        assert rel(y2, oracle.spmv(len(lens), 4000, rp, ci, va, xv2, acc)) <= TOL_SPMV and intact(vab, nnz)
+    S.close()
+
+
 def test_tolerance_stop_matches_oracle_cfg0(g0, cfg0):
     b, damp = cfg0["b"], cfg0["damp"]
     g0.S.set(accumulate=1)
