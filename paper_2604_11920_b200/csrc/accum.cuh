@@ -6,9 +6,10 @@
 //   MODE 1 "dd"  : every product is formed exactly (TwoProd by FMA) and added into an unevaluated
 //                  double-double (hi, lo) (Knuth TwoSum); partial sums of lanes / warps / blocks are
 //                  combined by a dd+dd addition and the total is rounded to fp64 ONCE.  The rounded
-//                  result is the correctly rounded exact sum (up to ~1e-10-probability ties), hence
-//                  independent of the order of summation, which is what makes the fixed-k iterate
-//                  reproducible at scale.
+//                  result is a faithful rounding of the exact sum, and the correctly rounded one unless the
+//                  exact sum lies within ~2^-100 relative of a rounding boundary (probability ~1e-14 * cond
+//                  per sum), hence independent of the order of summation in practice, which is what makes
+//                  the fixed-k iterate reproducible at scale (the tests assert it bitwise and record it).
 // This translation unit is compiled with --fmad=false: a fused multiply-add exists only where fma() is
 // written, so the error-free transformations below are not contracted away.
 #pragma once

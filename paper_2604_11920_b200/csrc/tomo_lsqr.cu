@@ -223,6 +223,8 @@ tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
   if (!h->part_dirty) return TOMO_OK;
   const int tb = 128;
   // one persistent CTA per SM, W warp ranges each: cost-balanced element split points at multiples of the tile size
+  // (fewer CTAs for small systems were measured slower: config 0 35 instead of 26 us per launch — the launch is
+  // bound by the serial tiles of a warp, not by the chain over CTA records)
   h->SG = h->sms;
   const int parts = h->SG * WC::W;
   const int gs = (parts + 1 + tb - 1) / tb;
@@ -1047,13 +1049,6 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "k4_ms") *out = h->k4_ms;
   else if (k == "k_launches") *out = h->k_launches;
   else if (k == "kernels_enqueued") *out = h->kernels_enqueued;
-  else if (k.rfind("cta_busy@", 0) == 0) {  // busy cycles of CTA <i> in the most recent sparse-product launch
-    const int i = atoi(k.c_str() + 9);
-    if (i < 0 || i >= h->SG) return TOMO_ERR_INVALID_ARG;
-    CtaRec r;
-    CK(cudaMemcpy(&r, h->cta_rec + i, sizeof(CtaRec), cudaMemcpyDeviceToHost));
-    *out = 16.0 * (double)r.pad;
-  }
   else if (k == "cta_busy_min" || k == "cta_busy_max" || k == "cta_busy_mean") {
     // busy cycles of the persistent CTAs in the most recent SpMV launch (load balance of the static split)
     std::vector<CtaRec> rec(h->SG);
