@@ -211,6 +211,8 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
     S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=args.compress)
     if args.row_cost is not None:
         S.set(row_cost=args.row_cost)
+    if args.pdl is not None:
+        S.set(pdl=args.pdl)
     b = b_host.cuda()
     x = torch.empty(n, dtype=torch.float64, device="cuda")
     lsmr = args.solver == "lsmr"
@@ -281,6 +283,83 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
         out["index_bytes"] = (S.info("compress_bytes_rows"), S.info("compress_bytes_cols"))
     S.close()
     return out
+
+
+def run_sharded(args) -> dict | None:
+    """`--shards P`: the configs[C] matrix cut into P nnz-balanced row blocks, solved by
+    tomo_lsqr_solve_sharded.  One process: all P blocks on this GPU (the exchange is the identity; measures what the
+    unrounded partials and the closing kernels cost).  Under torchrun with N ranks: P = N, rank r holds block r, the
+    exchange is an NCCL all-gather; the total work is fixed (strong scaling)."""
+    import numpy as np
+    import torch
+    import paper_2604_11920_b200 as tl
+    import tomogen
+    tl.load()
+    world, rank, local = (int(os.environ.get(k, d)) for k, d in (("WORLD_SIZE", "1"), ("RANK", "0"), ("LOCAL_RANK", "0")))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    s = tomogen.System(args.config)
+    m, n, nnz = s.dims.m, s.dims.n, s.dims.nnz
+    P = world if world > 1 else args.shards
+    rp = s.rowptr()
+    cuts = [0] + [int(np.searchsorted(rp, rp[-1] * q / P)) for q in range(1, P)] + [m]
+    mine = [rank] if world > 1 else list(range(P))
+    rp_d, ci_d, va_d = s.csr_cuda()
+    b_all = torch.from_numpy(s.rhs(0)).cuda()
+    blocks, bs = [], []
+    for q in mine:
+        a, c = cuts[q], cuts[q + 1]
+        e0, e1 = int(rp[a]), int(rp[c])
+        blocks.append(tl.TomoLsqr(c - a, n, (rp_d[a:c + 1] - e0).contiguous(), ci_d[e0:e1].clone(), va_d[e0:e1].clone()))
+        bs.append(b_all[a:c].clone())
+    del rp_d, ci_d, va_d
+    blocks[0].set(accumulate=args.accumulate, check_every=args.check_every)
+    cb = tl.make_allgather(dist, world) if world > 1 else None
+    x = torch.empty(n, dtype=torch.float64, device="cuda")
+    damp, atol, btol, max_iters = s.damp, s.solve["atol"], s.solve["btol"], s.solve["max_iters"]
+
+    def step():
+        return tl.tomo_lsqr_solve_sharded([B.h for B in blocks], bs, damp, atol, btol, max_iters, x, rank=rank, nranks=world, allgather=cb)
+
+    for _ in range(args.warmup):
+        step()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        e0.record()
+        its = sum(step().itn for _ in range(args.steps))
+        e1.record()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+    ab = algorithmic_bytes(m, n, nnz, 8)
+    extra = P * 16 * n * 2 + P * 16 * n  # the unrounded column pairs: written by every block, read once by the closing kernel
+    peak, peak_src = measured_peak_gbs()
+    return {"metric": METRIC, "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": workload_name(s), "row_blocks": P, "blocks_per_gpu": len(mine),
+                       "accumulate": "dd" if args.accumulate else "fast", "parallelism": f"row-sharded LSQR, {P} row blocks over {world} GPU(s)",
+                       "exchange": "NCCL all-gather of (hi, lo) partials" if world > 1 else "none (all blocks on one GPU)",
+                       "l2": "inputs larger than L2, no flush needed"},
+            "effective_gbs": (ab["iteration"] + extra) * its / (ms * 1e-3) / 1e9, "clocks": clk.summary(),
+            "roofline": {"bound": "hbm", "kernel": "k_wstream OP_K1S / OP_K2S over the row blocks + k_shard_combine (whole iteration, graph-less)",
+                         "achieved": (ab["iteration"] + extra) * its / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": (ab["iteration"] + extra) * its / (ms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src},
+            "gpu_launches": int(sum(B.info("kernels_enqueued") for B in blocks))}
 
 
 def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
@@ -448,6 +527,8 @@ def main():
     ap.add_argument("--vals", default="f64", choices=["f64", "f32"], help="storage type of the matrix values")
     ap.add_argument("--compress", type=int, default=0, choices=[0, 1], help="1: run-compressed index (NEXT-2), reported with its own byte count")
     ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
+    ap.add_argument("--pdl", type=int, default=None, choices=[0, 1], help="tuning: programmatic dependent launch between the kernels of an iteration")
+    ap.add_argument("--shards", type=int, default=0, help="NEXT-3: P row blocks solved by tomo_lsqr_solve_sharded (one GPU: all blocks local; torchrun: one block per rank)")
     ap.add_argument("--stub-step", dest="stub", action="store_true", help="TEST-ONLY: rank plumbing with a step that does no work (no GPU)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -458,7 +539,7 @@ def main():
         return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         sys.exit(relaunch_under_torchrun(args))
-    out = run_stub(args) if args.stub else run_ours(args)
+    out = run_stub(args) if args.stub else (run_sharded(args) if args.shards > 0 else run_ours(args))
     if out is not None:
         print(json.dumps(out), flush=True)
 

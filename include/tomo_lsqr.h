@@ -36,6 +36,7 @@
 #ifndef TOMO_LSQR_H_
 #define TOMO_LSQR_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -125,6 +126,25 @@ tomo_status_t tomo_lsqr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d
 tomo_status_t tomo_lsmr_solve_multi(tomo_lsqr_t h, int32_t nrhs, const double* d_B, double damp, double atol,
                                     double btol, int32_t max_iters, double* d_X, tomo_lsqr_result_t* res,
                                     void* cuda_stream);
+
+/* NEXT-3: row-sharded LSQR.  A = [A_1; ...; A_P] by row blocks in the global order "rank 0's
+ * blocks, rank 1's blocks, ..."; every block is an ordinary handle created on its own rows (m_p x n, all with the
+ * same n and value type, on this rank's device); b is split the same way (d_b[l] fp64[m_l]).  u and b are local to a
+ * block, v, w, x and the scalars are replicated: d_x fp64[n] is written in full on every rank.  Per iteration every
+ * block computes u^_p = A_p v - alpha u_p and the UNROUNDED (hi, lo) pairs of ||u^_p||^2 and of A_p^T u_p per column;
+ * two exchanges (16 bytes and 16 n bytes per block) gather them in block order and the sums are closed in that fixed
+ * order and rounded once: in double-double mode the iterates are bit for bit those of tomo_lsqr_solve on the whole
+ * matrix, in fast mode a deterministic sum in block order.  Options ("accumulate", "check_every") are taken from
+ * shards[0]; runs on the int32 index without CUDA graph.
+ * allgather (may be NULL iff nranks == 1): device all-gather supplied by the caller (e.g. NCCL through
+ * torch.distributed): every rank contributes `bytes` bytes at d_send, on return d_recv holds nranks * bytes with rank
+ * r's contribution at offset r * bytes; it must be ordered with `cuda_stream`; returns 0 on success.  The buffers
+ * belong to shards[0]. */
+typedef int (*tomo_allgather_fn)(void* ctx, const void* d_send, void* d_recv, size_t bytes, void* cuda_stream);
+tomo_status_t tomo_lsqr_solve_sharded(const tomo_lsqr_t* shards, int32_t nlocal, int32_t rank, int32_t nranks,
+                                      tomo_allgather_fn allgather, void* ctx, const double* const* d_b, double damp,
+                                      double atol, double btol, int32_t max_iters, double* d_x, tomo_lsqr_result_t* res,
+                                      void* cuda_stream);
 
 /* y = A x (transpose = 0: d_in fp64[n], d_out fp64[m]) or y = A^T x (transpose = 1: d_in fp64[m],
  * d_out fp64[n]) with the kernels the solver uses (the A^T product gathers over the CSC copy). */

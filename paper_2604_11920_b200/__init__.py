@@ -23,9 +23,13 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
     "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
-    "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values",
+    "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values", "tomo_lsqr_solve_sharded",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
 )
+
+
+# int allgather(void* ctx, const void* d_send, void* d_recv, size_t bytes, void* cuda_stream)
+ALLGATHER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
 
 
 class tomo_lsqr_result_t(ctypes.Structure):
@@ -62,6 +66,8 @@ def load() -> ctypes.CDLL:
     lib.tomo_lsmr_solve_multi.argtypes = lib.tomo_lsqr_solve_multi.argtypes
     lib.tomo_lsqr_spmv.argtypes = [vp, ci, vp, vp, vp]
     lib.tomo_lsqr_update_values.argtypes = [vp, vp, vp]
+    lib.tomo_lsqr_solve_sharded.argtypes = [ctypes.POINTER(vp), i32, i32, i32, ALLGATHER_FN, vp, ctypes.POINTER(vp), f64, f64, f64, i32, vp,
+                                            ctypes.POINTER(tomo_lsqr_result_t), vp]
     lib.tomo_lsqr_get_csc.argtypes = [vp, vp, vp, vp, vp]
     lib.tomo_lsqr_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.tomo_lsqr_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(f64)]
@@ -165,6 +171,55 @@ def tomo_lsqr_spmv(h, transpose, d_in, d_out, stream=None) -> None:
     st = load().tomo_lsqr_spmv(h, int(transpose), _ptr(d_in), _ptr(d_out), _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_spmv")
+
+
+class _RawBytes:
+    """A raw device buffer (address, length) as a CUDA-array-interface object, so that torch can wrap it without a copy."""
+
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def make_allgather(dist, world_size: int, device: str = "cuda"):
+    """The exchange of tomo_lsqr_solve_sharded on top of torch.distributed (marshalling only): wraps the two raw
+    buffers the library hands over as byte tensors and calls all_gather_into_tensor (NCCL on `cuda`; `cpu` wraps host
+    memory for the gloo test of this wrapper).  Returns the ctypes callback; keep a reference while it is in use."""
+    import torch
+
+    def wrap(ptr, nbytes):
+        if device == "cuda":
+            return torch.as_tensor(_RawBytes(ptr, nbytes), device="cuda")
+        import numpy as np
+        return torch.from_numpy(np.ctypeslib.as_array(ctypes.cast(ptr, ctypes.POINTER(ctypes.c_uint8)), shape=(nbytes,)))
+
+    def allgather(ctx, d_send, d_recv, nbytes, stream):
+        try:
+            send, recv = wrap(d_send, nbytes), wrap(d_recv, nbytes * world_size)
+            if device == "cuda":
+                ext = torch.cuda.ExternalStream(stream) if stream else torch.cuda.default_stream()
+                with torch.cuda.stream(ext):
+                    dist.all_gather_into_tensor(recv, send)
+            else:
+                dist.all_gather_into_tensor(recv, send)
+            return 0
+        except Exception:  # noqa: BLE001 - a C callback must not raise
+            return 1
+
+    return ALLGATHER_FN(allgather)
+
+
+def tomo_lsqr_solve_sharded(handles, d_bs, damp, atol, btol, max_iters, d_x, rank=0, nranks=1, allgather=None, stream=None) -> tomo_lsqr_result_t:
+    """handles / d_bs: this rank's row blocks and their right-hand sides, in order; allgather: make_allgather(...) if nranks > 1."""
+    nl = len(handles)
+    hs = (ctypes.c_void_p * nl)(*handles)
+    bs = (ctypes.c_void_p * nl)(*[_ptr(b) for b in d_bs])
+    res = tomo_lsqr_result_t()
+    cb = allgather if allgather is not None else ctypes.cast(None, ALLGATHER_FN)
+    st = load().tomo_lsqr_solve_sharded(hs, nl, rank, nranks, cb, None, bs, damp, atol, btol, max_iters, _ptr(d_x), ctypes.byref(res),
+                                        _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_solve_sharded")
+    return res
 
 
 def tomo_lsqr_update_values(h, d_vals, stream=None) -> None:

@@ -162,6 +162,22 @@ __device__ __forceinline__ double final_sum(const double2* partials, int count, 
   return a.value();
 }
 
+// the same, unrounded: the (hi, lo) pair of the total in thread 0 (sharded solve: the sum is closed after an exchange)
+template <int MODE>
+__device__ __forceinline__ double2 final_sum_pair(const double2* partials, int count, double2* slots) {
+  Acc<MODE> a;
+  a.zero();
+  for (int i = threadIdx.x; i < count; i += blockDim.x) {
+    Acc<MODE> o;
+    o.unpack(__ldcg(partials + i));
+    a.merge(o);
+  }
+  lanes_reduce<32, MODE>(a);
+  __syncthreads();
+  block_combine<MODE>(a, slots);
+  return a.pack();
+}
+
 // Publish this block's partial and find out whether it is the last block of the launch.
 __device__ __forceinline__ bool publish_and_ticket(double2* partials, double2 mine, unsigned int* ticket, int* s_flag) {
   if (threadIdx.x == 0) {

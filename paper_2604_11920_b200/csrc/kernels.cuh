@@ -30,12 +30,12 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
   __shared__ double2 s_slots[kWarps];
   __shared__ int s_flag;
   grid_dependency_wait();
-  if (VOP != VOP_INIT_U && sc->stop) return;
+  if (VOP != VOP_INIT_U && VOP != VOP_INIT_US && sc->stop) return;
   Acc<MODE> acc;
   acc.zero();
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (VOP == VOP_INIT_U) {
+  if (VOP == VOP_INIT_U || VOP == VOP_INIT_US) {
     for (int64_t i = i0; i < len; i += stride) {
       double b = in0[i];
       a0[i] = b;
@@ -94,8 +94,12 @@ __global__ void __launch_bounds__(kThreads) k_vec(const double* __restrict__ in0
   block_combine<MODE>(acc, s_slots);
   grid_launch_dependents();
   if (publish_and_ticket(partials, acc.pack(), &sc->ticket[1], &s_flag)) {
-    double total = final_sum<MODE>(partials, gridDim.x, s_slots);
+    const double2 pair = final_sum_pair<MODE>(partials, gridDim.x, s_slots);
     if (threadIdx.x == 0) {
+      Acc<MODE> t;
+      t.unpack(pair);
+      const double total = t.value();
+      if (VOP == VOP_INIT_US) reinterpret_cast<double2*>(a3)[0] = pair;
       if (VOP == VOP_INIT_U) tail_init_u(sc, total);
       if (VOP == VOP_K4) tail_k4(sc, total);
       if (VOP == VOP_K4_LSMR) tail_k4_lsmr(sc, total);

@@ -47,14 +47,18 @@ enum SpmvOp : int {
   OP_PLAIN = 0,   // y = A x                       (tomo_lsqr_spmv)
   OP_K1 = 1,      // u^ = A v - alpha u  , ||u^||^2 ; tail: beta, anorm
   OP_K2 = 2,      // v^ = A^T u - beta v , ||v^||^2 ; tail: alpha, rotations, estimates
-  OP_K2_INIT = 3  // v^ = A^T u          , ||v^||^2 ; tail: alpha_1, rhobar, phibar
+  OP_K2_INIT = 3, // v^ = A^T u          , ||v^||^2 ; tail: alpha_1, rhobar, phibar
+  // row-sharded solve (shard.cuh): one row block of A per launch, the sums over blocks are closed after an exchange
+  OP_K1S = 4,     // u^_p = A_p v - alpha u_p ; the block's ||u^_p||^2 as an unrounded (hi, lo) pair, no tail
+  OP_K2S = 5      // t_p = A_p^T u_p as UNROUNDED (hi, lo) pairs per column (y is a double2 array), no norm, no tail
 };
 
 enum VecOp : int {
   VOP_INIT_U = 0,  // u^ = b, ||b||^2 ; tail: beta_1
   VOP_INIT_VW = 1, // v = v^/alpha, w = v, x = 0
   VOP_K4 = 2,      // v = v^/alpha ; ddnorm partial ; x += t1 w ; w = v + t2 w ; tail: stop tests
-  VOP_K4_LSMR = 3  // v = v^/alpha ; hbar = h + f1 hbar ; x += f2 hbar ; h = v + f3 h ; ||x||^2 ; tail: stop tests
+  VOP_K4_LSMR = 3, // v = v^/alpha ; hbar = h + f1 hbar ; x += f2 hbar ; h = v + f3 h ; ||x||^2 ; tail: stop tests
+  VOP_INIT_US = 4  // sharded: u^_p = b_p ; ||b_p||^2 as an unrounded pair to a3[0..1], no tail
 };
 
 }  // namespace tomo

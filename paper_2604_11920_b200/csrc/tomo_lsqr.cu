@@ -18,6 +18,7 @@
 #include "kernels.cuh"
 #include "wstream.cuh"
 #include "compress.cuh"
+#include "shard.cuh"
 #include "multi.cuh"
 
 using namespace tomo;
@@ -96,6 +97,7 @@ struct tomo_lsqr_s {
   int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 320, pdl = 1, compress = 0;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, transpose_kernels_ms = 0, update_ms = 0, scratch_bytes = 0;
+  double2* sh_send = nullptr; double2* sh_recv = nullptr; int64_t sh_send_cap = 0, sh_recv_cap = 0;  // exchange buffers of the sharded solve
   void* pos = nullptr; bool pos_wide = false;   // CSR element -> CSC slot (built by the first tomo_lsqr_update_values)
   double k1_ms = 0, k2_ms = 0, k4_ms = 0, k_launches = 0;
   double kernels_enqueued = 0;  // cumulative count of this library's kernel launches (graph nodes included)
@@ -132,7 +134,7 @@ template <bool TR> struct WCOf { using type = WC; };
 template <> struct WCOf<true> { using type = WCT; };
 
 template <int MODE, typename VT, int OP, int FMT, bool TR>
-cudaError_t launch_wstream_t(const tomo_lsqr_s* h, const double* x, double* y, cudaStream_t st) {
+cudaError_t launch_wstream_t(const tomo_lsqr_s* h, const double* x, double* y, cudaStream_t st, Scalars* sc_shared = nullptr) {
   using C = typename WCOf<TR>::type;
   const Dir& d = h->dir[TR ? 1 : 0];
   auto kern = k_wstream<C, MODE, VT, OP, FMT>;
@@ -142,10 +144,10 @@ cudaError_t launch_wstream_t(const tomo_lsqr_s* h, const double* x, double* y, c
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = (h->pdl && OP != OP_PLAIN) ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = (h->pdl && OP != OP_PLAIN && OP != OP_K1S && OP != OP_K2S) ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kern, d.ptr, (const int32_t*)d.rid, d.idx, (const VT*)d.val, (const unsigned char*)d.cidx,
                             (const int64_t*)d.coff, h->nnz, d.nrows, (const int32_t*)d.erows, d.n_empty, x, y,
-                            (const int64_t*)d.wE, (const int32_t*)d.wR, h->cta_rec, h->sc, h->part_spmv);
+                            (const int64_t*)d.wE, (const int32_t*)d.wR, h->cta_rec, sc_shared ? sc_shared : h->sc, h->part_spmv);
 }
 
 // The > 48 KB dynamic shared memory opt-in of every k_wstream instantiation, on the CURRENT device (function
@@ -163,6 +165,10 @@ cudaError_t stream_attr_ops() {
   if ((e = stream_attr_one<WC, MODE, VT, OP_K1, FMT>()) != cudaSuccess) return e;
   if ((e = stream_attr_one<WCT, MODE, VT, OP_PLAIN, FMT>()) != cudaSuccess) return e;
   if ((e = stream_attr_one<WCT, MODE, VT, OP_K2, FMT>()) != cudaSuccess) return e;
+  if (FMT == 0) {  // the row-sharded solve runs on the int32 index
+    if ((e = stream_attr_one<WC, MODE, VT, OP_K1S, 0>()) != cudaSuccess) return e;
+    if ((e = stream_attr_one<WCT, MODE, VT, OP_K2S, 0>()) != cudaSuccess) return e;
+  }
   return stream_attr_one<WCT, MODE, VT, OP_K2_INIT, FMT>();
 }
 template <typename VT>
@@ -379,7 +385,7 @@ void free_handle(tomo_lsqr_s* h) {
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   for (int i = 0; i < 2; ++i) if (h->ev_poll[i]) cudaEventDestroy(h->ev_poll[i]);
   for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
-  cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals); cudaFree(h->pos);
+  cudaFree(h->colptr); cudaFree(h->rowind); cudaFree(h->cvals); cudaFree(h->pos); cudaFree(h->sh_send); cudaFree(h->sh_recv);
   cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->mH); cudaFree(h->msc); cudaFree(h->cta_rec8);
   cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->h_mpoll) cudaFreeHost(h->h_mpoll); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
@@ -982,6 +988,120 @@ extern "C" tomo_status_t tomo_lsqr_update_values(tomo_lsqr_t h, const void* d_va
   if ((uintptr_t)d_vals & 15u) return TOMO_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   return h->vt == TOMO_VAL_F64 ? update_values_t<double>(h, (const double*)d_vals, st) : update_values_t<float>(h, (const float*)d_vals, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-3: row-sharded LSQR (shard.cuh)
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+template <int MODE, typename VT>
+tomo_status_t solve_sharded_t(tomo_lsqr_s* const* sh, int nlocal, int rank, int nranks, tomo_allgather_fn allgather, void* ctx,
+                              const double* const* d_b, double damp, double atol, double btol, int32_t max_iters, double* d_x,
+                              tomo_lsqr_result_t* res, cudaStream_t st) {
+  tomo_lsqr_s* h0 = sh[0];
+  const int64_t n = h0->n;
+  const int P = nlocal * nranks;
+  // exchange buffers: per block one norm pair followed by n column pairs; send = my nlocal blocks, recv = all P blocks
+  const int64_t per = n + 1;
+  if (h0->sh_send_cap < per * nlocal) {
+    cudaFree(h0->sh_send); h0->sh_send = nullptr; h0->sh_send_cap = 0;
+    CK(cudaMalloc(&h0->sh_send, sizeof(double2) * per * nlocal));
+    h0->sh_send_cap = per * nlocal;
+  }
+  if (nranks > 1 && h0->sh_recv_cap < per * P) {
+    cudaFree(h0->sh_recv); h0->sh_recv = nullptr; h0->sh_recv_cap = 0;
+    CK(cudaMalloc(&h0->sh_recv, sizeof(double2) * per * P));
+    h0->sh_recv_cap = per * P;
+  }
+  // layout: norms [blocks], then column pairs [blocks][n]; with one rank the send buffer is the gathered buffer
+  double2* norm_send = h0->sh_send;
+  double2* t_send = h0->sh_send + nlocal;
+  double2* norm_all = nranks > 1 ? h0->sh_recv : norm_send;
+  double2* t_all = nranks > 1 ? h0->sh_recv + P : t_send;
+  auto exchange = [&](double2* send, double2* recv, int64_t pairs_per_rank) -> tomo_status_t {
+    if (nranks == 1) return TOMO_OK;
+    if (allgather(ctx, send, recv, (size_t)pairs_per_rank * sizeof(double2), (void*)st) != 0) return TOMO_ERR_CUDA;
+    return TOMO_OK;
+  };
+  for (int l = 0; l < nlocal; ++l) { tomo_status_t rc = rebuild_partitions(sh[l], st); if (rc != TOMO_OK) return rc; }
+
+  Scalars* hs = h0->h_sc;
+  memset(hs, 0, sizeof(Scalars));
+  hs->damp = damp; hs->atol = atol; hs->btol = btol; hs->max_iters = max_iters; hs->cs2 = -1.0; hs->solver = 0;
+  CK(cudaMemcpyAsync(h0->sc, hs, sizeof(Scalars), cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(h0->x, 0, sizeof(double) * n, st));
+  Scalars* sc = h0->sc;
+  const int gv = vec_blocks(h0, n);
+  auto k1s = [&](int l) { launch_wstream_t<MODE, VT, OP_K1S, 0, false>(sh[l], h0->v, sh[l]->u, st, sc);
+                          cudaMemcpyAsync(norm_send + l, sh[l]->part_spmv + sh[l]->SG, sizeof(double2), cudaMemcpyDeviceToDevice, st); };
+  auto k2s = [&](int l) { launch_wstream_t<MODE, VT, OP_K2S, 0, true>(sh[l], sh[l]->u, reinterpret_cast<double*>(t_send + (int64_t)l * n), st, sc); };
+  // a1: beta_1 = ||b||, u^ = b, v^ = A^T u, alpha_1, w = v
+  for (int l = 0; l < nlocal; ++l)
+    k_vec<MODE, VOP_INIT_US><<<vec_blocks(sh[l], sh[l]->m), kThreads, 0, st>>>(d_b[l], sh[l]->u, nullptr, nullptr,
+                                                                             reinterpret_cast<double*>(norm_send + l), sh[l]->m, sc, sh[l]->part_vec);
+  { tomo_status_t rc = exchange(norm_send, norm_all, nlocal); if (rc != TOMO_OK) return rc; }
+  k_shard_norm<MODE, 0><<<1, 32, 0, st>>>(norm_all, P, sc);
+  for (int l = 0; l < nlocal; ++l) k2s(l);
+  { tomo_status_t rc = exchange(t_send, t_all, (int64_t)nlocal * n); if (rc != TOMO_OK) return rc; }
+  k_shard_combine<MODE, true><<<gv, 256, 0, st>>>(t_all, P, n, h0->v, sc, h0->part_vec);
+  k_vec<MODE, VOP_INIT_VW><<<gv, kThreads, 0, st>>>(nullptr, h0->v, h0->w, nullptr, nullptr, n, sc, h0->part_vec);
+  CK(cudaGetLastError());
+  double launches = 4.0 + 2.0 * nlocal;
+  const int k = h0->check_every;
+  bool stopped = false;
+  for (int it = 0; it < max_iters && !stopped; ++it) {
+    for (int l = 0; l < nlocal; ++l) k1s(l);
+    { tomo_status_t rc = exchange(norm_send, norm_all, nlocal); if (rc != TOMO_OK) return rc; }
+    k_shard_norm<MODE, 1><<<1, 32, 0, st>>>(norm_all, P, sc);
+    for (int l = 0; l < nlocal; ++l) k2s(l);
+    { tomo_status_t rc = exchange(t_send, t_all, (int64_t)nlocal * n); if (rc != TOMO_OK) return rc; }
+    k_shard_combine<MODE, false><<<gv, 256, 0, st>>>(t_all, P, n, h0->v, sc, h0->part_vec);
+    k_vec<MODE, VOP_K4><<<gv, kThreads, 0, st>>>(nullptr, h0->v, h0->w, h0->x, nullptr, n, sc, h0->part_vec);
+    launches += 3.0 + 2.0 * nlocal;
+    if ((it + 1) % k == 0 || it + 1 == max_iters) {  // host poll (every rank sees the same replicated stop flag)
+      CK(cudaGetLastError());
+      CK(cudaMemcpyAsync(&h0->h_poll[0], &sc->itn, sizeof(PollWord), cudaMemcpyDeviceToHost, st));
+      CK(cudaStreamSynchronize(st));
+      if (h0->h_poll[0].stop) stopped = true;
+    }
+  }
+  h0->kernels_enqueued += launches;
+  CK(cudaMemcpyAsync(d_x, h0->x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(hs, sc, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (res) {
+    res->itn = hs->itn; res->istop = hs->istop;
+    res->r1norm = hs->r1norm; res->r2norm = hs->r2norm; res->arnorm = hs->arnorm;
+    res->anorm = hs->anorm; res->acond = hs->acond; res->xnorm = hs->xnorm;
+  }
+  return TOMO_OK;
+}
+
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_solve_sharded(const tomo_lsqr_t* shards, int32_t nlocal, int32_t rank, int32_t nranks,
+                                                 tomo_allgather_fn allgather, void* ctx, const double* const* d_b, double damp,
+                                                 double atol, double btol, int32_t max_iters, double* d_x, tomo_lsqr_result_t* res,
+                                                 void* cuda_stream) {
+  if (!shards || nlocal < 1 || nlocal > 64 || nranks < 1 || rank < 0 || rank >= nranks || !d_b || !d_x) return TOMO_ERR_INVALID_ARG;
+  if (nranks > 1 && !allgather) return TOMO_ERR_INVALID_ARG;
+  tomo_lsqr_s* h0 = shards[0];
+  tomo_status_t rc = check_solve_args(h0, damp, atol, btol, max_iters);
+  if (rc != TOMO_OK) return rc;
+  if (!is_device_ptr(d_x)) return TOMO_ERR_NOT_DEVICE_PTR;
+  for (int l = 0; l < nlocal; ++l) {
+    const tomo_lsqr_s* h = shards[l];
+    if (!h || h->n != h0->n || h->vt != h0->vt || h->device != h0->device) return TOMO_ERR_INVALID_ARG;
+    if (!d_b[l]) return TOMO_ERR_INVALID_ARG;
+    if (!is_device_ptr(d_b[l])) return TOMO_ERR_NOT_DEVICE_PTR;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h0->vt == TOMO_VAL_F64)
+    return h0->accumulate ? solve_sharded_t<1, double>(shards, nlocal, rank, nranks, allgather, ctx, d_b, damp, atol, btol, max_iters, d_x, res, st)
+                          : solve_sharded_t<0, double>(shards, nlocal, rank, nranks, allgather, ctx, d_b, damp, atol, btol, max_iters, d_x, res, st);
+  return h0->accumulate ? solve_sharded_t<1, float>(shards, nlocal, rank, nranks, allgather, ctx, d_b, damp, atol, btol, max_iters, d_x, res, st)
+                        : solve_sharded_t<0, float>(shards, nlocal, rank, nranks, allgather, ctx, d_b, damp, atol, btol, max_iters, d_x, res, st);
 }
 
 extern "C" tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const double* d_in, double* d_out, void* cuda_stream) {

@@ -171,9 +171,13 @@ __device__ __forceinline__ Acc<MODE> acc_of(double2 p) {
 template <int MODE, int OP>
 __device__ __forceinline__ void finish_row_with(Acc<MODE> sum, double yo, double* __restrict__ y, int64_t r, double c,
                                                 double sy, Acc<MODE>& nsq) {
+  if (OP == OP_K2S) {  // the unrounded partial column sum of this row block: closed after the exchange (shard.cuh)
+    reinterpret_cast<double2*>(y)[r] = sum.pack();
+    return;
+  }
   double yn;
-  if (OP == OP_K1 || OP == OP_K2) {
-    if (OP == OP_K1) yo = yo * sy;
+  if (OP == OP_K1 || OP == OP_K2 || OP == OP_K1S) {
+    if (OP == OP_K1 || OP == OP_K1S) yo = yo * sy;
     if (MODE == 0) {
       yn = fma(c, yo, sum.value());
     } else {
@@ -287,7 +291,7 @@ __device__ __forceinline__ int64_t row_number(const WCtx& cx, int k) { return cx
 // runs on.  One copy in the code, called from a non-unrolled loop.
 template <int MODE, int OP>
 __device__ __forceinline__ void slow_step(WSweep<MODE>& st, const WCtx& cx, double v, double x, int base) {
-  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
+  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2 || OP == OP_K1S);
   const int lane = threadIdx.x & 31;
   const int hi = min(base + 32, cx.len);
   const int pos = base + lane;
@@ -370,7 +374,7 @@ __device__ __forceinline__ void slow_step(WSweep<MODE>& st, const WCtx& cx, doub
 template <int MODE, int OP, bool SCALE_X>
 __device__ __forceinline__ void consume_round(WSweep<MODE>& st, const WCtx& cx, double (&vv)[8], double (&xx)[8], int pos0,
                                               double sx) {
-  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
+  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2 || OP == OP_K1S);
   const int lane = threadIdx.x & 31;
   if (SCALE_X) {
 #pragma unroll
@@ -444,8 +448,8 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   constexpr int TILE = CFG::TILE, NS = CFG::NS, W = CFG::W, RPT = CFG::RPT;
   using SM = WSmem<CFG, VT, FMT>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2);
-  constexpr bool SCALE_X = (OP == OP_K2 || OP == OP_K2_INIT);
+  constexpr bool NEEDS_Y = (OP == OP_K1 || OP == OP_K2 || OP == OP_K1S);
+  constexpr bool SCALE_X = (OP == OP_K2 || OP == OP_K2_INIT || OP == OP_K2S);
 
   const int lane = threadIdx.x & 31, warp = uni((int)(threadIdx.x >> 5));
   const long long t_start = clock64();
@@ -555,9 +559,10 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
       if (blockIdx.x == 0 && threadIdx.x == 0) tail_k2(sc, 0.0);
       skip = true;
     }
-    if (OP == OP_K1) { c = -sc->alpha; sy = sc->rbeta; }
+    else if (OP == OP_K2S && sc->beta_zero) skip = true;  // the combine kernel runs the scalar step
+    if (OP == OP_K1 || OP == OP_K1S) { c = -sc->alpha; sy = sc->rbeta; }
     if (OP == OP_K2) { c = -sc->beta; sx = sc->rbeta; }
-    if (OP == OP_K2_INIT) { sx = sc->rbeta; }
+    if (OP == OP_K2_INIT || OP == OP_K2S) { sx = sc->rbeta; }
   }
   if (skip) {  // drain the copies already requested (shared memory must not be written after the CTA exits)
     for (int t = 0; t < NS && t < ntiles; ++t) mbar_wait(my_bar + (t % NS), 0);
@@ -749,7 +754,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
     }
     lanes_reduce<32, MODE>(extra);
   }
-  if (OP == OP_PLAIN) {
+  if (OP == OP_PLAIN || OP == OP_K2S) {
     if (threadIdx.x == 0) sc->ticket[0] = 0u;
     return;
   }
@@ -764,6 +769,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   if (threadIdx.x == 0) {
     Acc<MODE> tot = acc_of<MODE>(s_slots[0]);
     for (int i = 1; i < W; ++i) tot.merge(acc_of<MODE>(s_slots[i]));
+    if (OP == OP_K1S) partials[gridDim.x] = tot.pack();  // this row block's ||u^_p||^2, unrounded: summed over blocks after the exchange
     const double total = tot.value();
     if (OP == OP_K1) tail_k1(sc, total);
     if (OP == OP_K2) tail_k2(sc, total);
