@@ -259,7 +259,7 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
             ms, its, launches = aggregate_over_ranks(dist, ms, its, launches, device="cuda")
         return ms, its, launches
 
-    out = {"m": m, "n": n, "nnz": nnz, "nrhs": nrhs, "vbytes": vbytes, "create_wall_ms": create_wall_ms,
+    out = {"m": m, "n": n, "nnz": nnz, "nrhs": nrhs, "vbytes": vbytes, "create_wall_ms": create_wall_ms, "accumulate": args.accumulate,
            "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms")}
     with ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) as clk:
         out["ms"], out["its"], out["launches"] = timed(step_device)
@@ -378,6 +378,18 @@ def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
     kern = ("k_wstream (K1: A v - alpha u + norm over CSR; K2: A^T u - beta v + norm over CSC), mean of the two launches of an iteration"
             if nrhs == 1 else
             "k_spmm8 (the same two products on len x 8 blocks, 8 right-hand sides per pass), mean of the two launches of a block iteration")
+    if nrhs > 1 and r.get("accumulate", 1) == 1:
+        # dd block solve: bound by the fp64 pipe, not by HBM.  Work = 10 fp64 instructions per (nonzero, side)
+        # (TwoProd 2 + TwoSum 6 + 2 error adds; an FMA counts once); peak = 148 SMs x 64 fp64 lanes per clock x the SM's
+        # maximum clock (B200: 40 TFLOP/s fp64 = 64 FMA lanes per SM and clock).
+        sm_max = (r.get("clocks") or {}).get("sm_max_mhz") or 1965.0
+        peak_t = 148 * 64 * sm_max * 1e6 / 1e12
+        ach_t = 10.0 * nnz * nrhs * 2 / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e12
+        return {"bound": "alu", "kernel": kern, "achieved": ach_t, "peak": peak_t, "unit": "TFLOP/s", "frac": ach_t / peak_t,
+                "peak_source": "derived: 148 SMs x 64 fp64 lanes/clk x sm_max_mhz (fp64 lane-instructions/s, FMA counted once)",
+                "work_per_launch": 10.0 * nnz * nrhs, "traffic": None,
+                "hbm_stream_gbs": achieved, "hbm_stream_frac_of_measured": achieved / peak, "bytes_per_launch_pair": spmv_bytes,
+                "k1_us": r["k1_us"], "k2_us": r["k2_us"], "k4_us": r["k4_us"]}
     return {"bound": "hbm", "kernel": kern, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
             "algorithmic_bytes_per_launch": spmv_bytes / 2, "byte_count": note, "peak_source": peak_src,
             "frac_of_8TBs": achieved / 8000.0, "bytes_per_launch_pair": spmv_bytes,
@@ -433,7 +445,8 @@ def run_ours(args) -> dict | None:
 
     peak, peak_src = measured_peak_gbs()
     rf = roofline_of(r, peak, peak_src, args.compress)
-    rf["traffic"], rf["traffic_source"] = ncu_traffic_bytes(args.config, nrhs)
+    if rf["bound"] == "hbm":
+        rf["traffic"], rf["traffic_source"] = ncu_traffic_bytes(args.config, nrhs)
     ab = algorithmic_bytes(m, n, nnz, vbytes) if nrhs == 1 else block_bytes(m, n, nnz, nrhs, vbytes)
     # bytes moved per second by the whole step: single side per iteration, block solve per BLOCK iteration (its / nrhs)
     eff = ab["iteration"] * (its / nrhs) / world / (ms * 1e-3) / 1e9

@@ -13,7 +13,8 @@
 //     barrier, no producer and no resolver warp between the first and the last element of a launch.
 //   * A tile is consumed in rounds of 256 elements (eight 32-element steps): the round's matrix entries go
 //     to registers and all eight gathers of x are issued at once; the gathers of round r+1 are in flight
-//     while round r is multiplied and summed (two register sets), which hides the L2 latency of the gather.
+//     while round r is multiplied and summed (two register sets), which hides the L2 latency of the gather; the
+//     values are read from the ring when the round is summed.
 //   * The per-lane accumulator of the open row lives across rounds and tiles; a warp reduction happens once
 //     per row, where the row ends.  A round that lies inside one row is eight exact products and a TwoSum
 //     tree (`mac8`); a round with a row end goes step by step; a step with several row ends (short rows:
@@ -28,8 +29,8 @@
 //     rows, rid = their row numbers) and lists them; the kernel gives them y_r <- c y_r in a side pass.
 //   * FMT 1 (run-compressed index; structure from Eq. 5 P:69-71 and the
 //     depth-fastest ordering Eq. 7): instead of one int32 per element the tile carries one bit per
-//     element ("continues a run of consecutive indices") and one int32 per run head (a head is forced at
-//     every 32-element step); the lane rebuilds its index with a popc / find-leading-one and one shared load.
+//     element ("starts a run of consecutive indices") and one int32 per run head (a head is forced at every
+//     32-element step); the lane rebuilds its index with one popc and one shared load (compress.cuh).
 // Every assignment (ranges, tiles, rounds, reduction trees) is static, so results are bitwise reproducible in
 // both accumulation modes; in dd mode they are moreover independent of all of it (DESIGN.md R-dd).
 #pragma once
