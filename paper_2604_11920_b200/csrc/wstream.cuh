@@ -64,6 +64,7 @@ struct CtaRec {        // what a warp (shared memory) or a CTA (global memory) l
 };
 
 constexpr int kBig = 0x3fffffff;  // "beyond the range" for relative element offsets
+constexpr int kPendRows = 4;      // finished rows whose per-lane partials wait in shared memory for one common reduction
 
 template <typename CFG, typename VT, int FMT>
 struct WSmem {
@@ -75,7 +76,8 @@ struct WSmem {
   static constexpr size_t kBars = 8 * CFG::NS * CFG::W;
   static constexpr size_t kRec = sizeof(CtaRec) * CFG::W;
   static constexpr size_t kSlots = sizeof(double2) * CFG::W + 16;
-  static constexpr size_t kTotal = kWarp * CFG::W + kBars + kRec + kSlots;
+  static constexpr size_t kPendWarp = sizeof(double2) * 32 * kPendRows + 16 * kPendRows;  // batched row ends (close_row)
+  static constexpr size_t kTotal = kWarp * CFG::W + kBars + kRec + kSlots + kPendWarp * CFG::W;
   static_assert(kStage % 16 == 0 && kIdx % 16 == 0, "bulk copies need 16-byte aligned destinations");
 };
 
@@ -254,11 +256,13 @@ struct WSweep {
   int next_b;        // relative offset where the open row ends (>= len: behind the range)
   int wbase;         // first row of the register window
   int S, S2;         // window: relative starts of rows wbase + lane and wbase + 32 + lane (kBig beyond row R1)
+  int np;            // rows waiting in the pend buffer
   bool started;      // the open row starts inside this range
 };
 
 struct WCtx {        // uniform, read-only
   const int64_t* ptr; const int32_t* rid; double* y; int64_t E0; int R0, R1, len; double c, sy;
+  double2* pend;     // per warp: [kPendRows][32] per-lane partials of finished rows, then [kPendRows] {old y, row number}
 };
 
 __device__ __forceinline__ int win_load(const WCtx& cx, int rbase) {
@@ -286,6 +290,48 @@ __device__ __forceinline__ void win_advance(ST& st, const WCtx& cx) {
 }
 __device__ __forceinline__ int64_t row_number(const WCtx& cx, int k) { return cx.rid ? (int64_t)cx.rid[k] : (int64_t)k; }
 
+// The rows that ended since the last flush: their per-lane partials sit in shared memory, [slot][lane].  Eight lanes per
+// row add four partials each (lane q takes lanes q, q+8, q+16, q+24: conflict-free), three butterfly steps close the
+// sum, the first lane of each group finishes its row.  One reduction for kPendRows rows instead of one (5 shuffle
+// steps + the finish code in ONE lane) per row.
+template <int MODE, int OP>
+__device__ __forceinline__ void flush_rows(WSweep<MODE>& st, const WCtx& cx) {
+  const int lane = threadIdx.x & 31;
+  __syncwarp();
+  const int k = lane >> 3, q = lane & 7;
+  const double2* p = cx.pend + k * 32 + q;
+  Acc<MODE> a = acc_of<MODE>(p[0]);
+#pragma unroll
+  for (int i = 1; i < 4; ++i) a.merge(acc_of<MODE>(p[8 * i]));
+#pragma unroll
+  for (int off = 1; off < 8; off <<= 1) {
+    double2 o = a.pack();
+    o.x = __shfl_xor_sync(0xffffffffu, o.x, off);
+    o.y = __shfl_xor_sync(0xffffffffu, o.y, off);
+    a.merge(acc_of<MODE>(o));
+  }
+  if (q == 0 && k < st.np) {
+    const double2 meta = cx.pend[32 * kPendRows + k];  // {old y, row number}
+    finish_row_with<MODE, OP>(a, meta.x, cx.y, row_number(cx, (int)__double_as_longlong(meta.y)), cx.c, cx.sy, st.nsq);
+  }
+  __syncwarp();
+  st.np = 0;
+}
+
+// the open row ends here: st.acc holds its per-lane partials
+template <int MODE, int OP>
+__device__ __forceinline__ void close_row(WSweep<MODE>& st, const WCtx& cx) {
+  const int lane = threadIdx.x & 31;
+  if (!st.started) {  // the row that was open at the range start: its sum goes to the warp's record (once per range)
+    lanes_reduce<32, MODE>(st.acc);
+    if (lane == 0) { st.h_val = st.acc.pack(); st.h_state = 2; }
+    return;
+  }
+  cx.pend[st.np * 32 + lane] = st.acc.pack();
+  if (lane == 0) cx.pend[32 * kPendRows + st.np] = make_double2(st.yold, __longlong_as_double((long long)st.cur));
+  if (++st.np == kPendRows) flush_rows<MODE, OP>(st, cx);
+}
+
 // One 32-element step [base, base+32) in which the open row ends (base < next_b <= base + 32): close it, then
 // give the remaining lanes' products to the rows that follow; rows that end inside the step are reduced
 // (segmented, 5 shuffle steps whatever their number) and finished, the last one becomes the open row if it
@@ -300,11 +346,7 @@ __device__ __forceinline__ void slow_step(WSweep<MODE>& st, const WCtx& cx, doub
   {
     const bool mine = pos < st.next_b;
     st.acc.mac(mine ? v : 0.0, mine ? x : 0.0);  // other lanes add an exact zero
-    lanes_reduce<32, MODE>(st.acc);
-    if (lane == 0) {
-      if (st.started) finish_row_with<MODE, OP>(st.acc, st.yold, cx.y, row_number(cx, st.cur), cx.c, cx.sy, st.nsq);
-      else { st.h_val = st.acc.pack(); st.h_state = 2; }
-    }
+    close_row<MODE, OP>(st, cx);
     st.acc.zero();
   }
   const int lo = st.next_b;
@@ -405,11 +447,7 @@ __device__ __forceinline__ void consume_round(WSweep<MODE>& st, const WCtx& cx, 
           accB.mac(first ? 0.0 : vv[u], first ? 0.0 : xx[u]);
         }
       }
-      lanes_reduce<32, MODE>(st.acc);
-      if (lane == 0) {
-        if (st.started) finish_row_with<MODE, OP>(st.acc, st.yold, cx.y, row_number(cx, st.cur), cx.c, cx.sy, st.nsq);
-        else { st.h_val = st.acc.pack(); st.h_state = 2; }
-      }
+      close_row<MODE, OP>(st, cx);
       st.acc = accB;
       st.started = true;
       if (pe >= cx.len) { st.next_b = kBig; return; }  // the range ends with this row
@@ -460,6 +498,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   CtaRec* s_rec = reinterpret_cast<CtaRec*>(smem_raw + SM::kWarp * W + SM::kBars);
   double2* s_slots = reinterpret_cast<double2*>(smem_raw + SM::kWarp * W + SM::kBars + SM::kRec);
   int* s_flag = reinterpret_cast<int*>(s_slots + W);
+  unsigned char* s_pend = smem_raw + SM::kWarp * W + SM::kBars + SM::kRec + SM::kSlots;
 
   // ---- prologue that depends on nothing the previous kernel writes: barriers, split points, first copies ----
   if (lane == 0) {
@@ -471,6 +510,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   const int gw = blockIdx.x * W + warp;
   WCtx cx;
   cx.ptr = ptr; cx.rid = rid; cx.y = y;
+  cx.pend = reinterpret_cast<double2*>(s_pend + (size_t)warp * SM::kPendWarp);
   cx.E0 = uni(wE[gw]);
   const int64_t E1 = uni(wE[gw + 1]);
   cx.R0 = uni(wR[gw]); cx.R1 = uni(wR[gw + 1]);
@@ -501,6 +541,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   auto issue_tile = [&](int t, bool refill) {
     const int s = t % NS;
     if (FMT == 0 && t != ntiles - 1) {  // a full tile: constant sizes, nothing but the two copies
+      __syncwarp();
       if (elect_one()) {
         if (refill) fence_proxy_async();
         const uint32_t dst = ring_a + (uint32_t)s * (uint32_t)SM::kStage, bar = bar_a + 8u * (uint32_t)s;
@@ -545,7 +586,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
 
   WSweep<MODE> st;
   st.acc.zero(); st.nsq.zero();
-  st.yold = 0.0; st.h_val = make_double2(0.0, 0.0); st.h_state = 0;
+  st.yold = 0.0; st.h_val = make_double2(0.0, 0.0); st.h_state = 0; st.np = 0;
   st.wbase = cx.R0;
   st.S = win_load(cx, cx.R0);
   st.S2 = win_load(cx, cx.R0 + 32);
@@ -649,6 +690,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   // The row still open at the end of the range continues in the next range.  The last row that starts in the
   // range is R1 - 1 (or, if none starts, the row that was open at the range start); it ends at ptr[R1] >= E1 and
   // is open iff ptr[R1] > E1.
+  if (st.np > 0) flush_rows<MODE, OP>(st, cx);  // finished rows still waiting for their reduction
   if (cx.len > 0) {
     const bool open = ptr[cx.R1] > E1;
     if (open) {
