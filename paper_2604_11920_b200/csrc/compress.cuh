@@ -13,10 +13,10 @@
 //     TILE/8 bytes   head bits, one 32-bit word per 32-element step: bit i = "element i starts a run":
 //                    i == 0 (a head is forced at every step, so a step decodes without looking back) or
 //                    idx[e] != idx[e-1] + 1
-//     4 bytes per head: idx[e] - i for every head, in element order (biased by its position i in the step, so
-//                    that the lane adds only its own lane number); padded to 16 bytes.
+//     4 bytes per head: idx[e] - i + 32 for every head, in element order (biased by its position i in the step, so
+//                    that the lane adds only its own lane number, and by 32 to stay non-negative); padded to 16 bytes.
 // Decoding (k_wstream, FMT 1): r = popc(H & lanes <= mine) counts the heads up to and including mine, the last
-// of them is my run's head: index = heads[heads before this step + r - 1] + lane.  One popc, one shared load.
+// of them is my run's head: index = heads[heads before this step + r - 1] - 32 + lane.  One popc, one shared load.
 // Runs may cross row boundaries: row membership comes from the row pointers, not from the index stream.
 #pragma once
 #include <cuda_runtime.h>
@@ -60,7 +60,7 @@ __global__ void k_cz_fill(const int32_t* __restrict__ idx, int64_t nnz, int64_t 
       if (e < nnz) { c = idx[e]; cont = (lane != 0) && (c == idx[e - 1] + 1); }
       const unsigned H = __ballot_sync(0xffffffffu, !cont);
       if (lane == 0) flags[s] = H;
-      if (!cont) heads[hb + __popc(H & ((1u << lane) - 1u))] = c - lane;
+      if (!cont) heads[hb + __popc(H & ((1u << lane) - 1u))] = c - lane + 32;
       hb += __popc(H);
     }
     // padding words of the record stay unwritten: they are never read (only copied)

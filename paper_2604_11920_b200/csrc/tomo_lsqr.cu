@@ -975,6 +975,10 @@ tomo_status_t update_values_t(tomo_lsqr_s* h, const VT* d_vals, cudaStream_t st)
   if (e == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess) h->update_ms = ms;
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   if (e != cudaSuccess) return cuda_fail(e, "value refresh");
+  if (h->vals != (const void*)d_vals) {  // the captured graphs hold the old pointer as a kernel argument
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    if (h->mgexec) { cudaGraphExecDestroy(h->mgexec); h->mgexec = nullptr; }
+  }
   h->vals = d_vals;
   h->dir[0].val = d_vals;
   return TOMO_OK;

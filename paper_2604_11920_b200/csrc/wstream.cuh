@@ -518,19 +518,20 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
   const int ntiles = (cx.len + TILE - 1) / TILE;
   const uint64_t policy = l2_evict_first_policy();
 
-  // FMT 1: byte offsets of the tile records, a register window of 32 (+1) entries refilled as the tiles go by
+  // FMT 1: the tile records are issued in order, so a running byte position and a register window of 32 record
+  // SIZES (refilled as the tiles go by) is all the bookkeeping the index stream needs
   const int64_t tile0 = cx.E0 / TILE;
-  int64_t coff_w = 0, coff_w1 = 0;  // coff[tile0 + cbase + lane], coff[tile0 + cbase + lane + 1]
+  uint32_t csize_w = 0;  // bytes of the record of tile cbase + lane
   int cbase = 0;
-  auto coff_load = [&](int base) {
+  const unsigned char* cpos = cidx;
+  auto csize_load = [&](int base) {
     if (FMT == 1) {
       const int t = base + lane;
-      coff_w = (t <= ntiles) ? coff[tile0 + t] : 0;
-      coff_w1 = (t + 1 <= ntiles) ? coff[tile0 + t + 1] : coff_w;
+      csize_w = (t < ntiles) ? (uint32_t)(coff[tile0 + t + 1] - coff[tile0 + t]) : 0u;
       cbase = base;
     }
   };
-  if (FMT == 1 && ntiles > 0) coff_load(0);
+  if (FMT == 1 && ntiles > 0) { csize_load(0); cpos = cidx + uni(coff[tile0]); }
 
   auto stage_ptr = [&](int s) { return my_ring + (size_t)s * SM::kStage; };
   // one lane requests tile t into stage t % NS (all lanes call, converged; every operand is warp-uniform).
@@ -551,6 +552,21 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
       }
       return;
     }
+    if (FMT == 1 && t - cbase >= 32) csize_load(t);
+    const uint32_t crec = (FMT == 1) ? (uint32_t)__shfl_sync(0xffffffffu, csize_w, t - cbase) : 0u;
+    const unsigned char* csrc = cpos;
+    if (FMT == 1) cpos += crec;
+    if (FMT == 1 && t != ntiles - 1) {  // a full tile of the run-compressed stream: the record (variable size) and the values
+      __syncwarp();
+      if (elect_one()) {
+        if (refill) fence_proxy_async();
+        const uint32_t dst = ring_a + (uint32_t)s * (uint32_t)SM::kStage, bar = bar_a + 8u * (uint32_t)s;
+        mbar_arrive_expect_tx_a(bar, crec + (uint32_t)(TILE * sizeof(VT)));
+        bulk_g2s_a(dst, csrc, crec, bar, policy);
+        bulk_g2s_a(dst + (uint32_t)SM::kIdx, val0 + (size_t)t * TILE, (uint32_t)(TILE * sizeof(VT)), bar, policy);
+      }
+      return;
+    }
     const int64_t e = cx.E0 + (int64_t)t * TILE;
     unsigned char* st_base = stage_ptr(s);
     int cnt4 = TILE;
@@ -562,20 +578,14 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
         if (FMT == 0) reinterpret_cast<int32_t*>(st_base)[cnt4 + lane] = idx[e + cnt4 + lane];
       }
     }
-    int64_t c0 = 0, c1 = 0;
-    if (FMT == 1) {
-      if (t - cbase >= 32) coff_load(t);
-      c0 = __shfl_sync(0xffffffffu, coff_w, t - cbase);
-      c1 = __shfl_sync(0xffffffffu, coff_w1, t - cbase);
-    }
     __syncwarp();
     if (elect_one()) {
       if (refill) fence_proxy_async();
       const uint32_t bv = (uint32_t)cnt4 * (uint32_t)sizeof(VT);
-      const uint32_t bi = (FMT == 0) ? (uint32_t)cnt4 * 4u : (uint32_t)(c1 - c0);
+      const uint32_t bi = (FMT == 0) ? (uint32_t)cnt4 * 4u : crec;
       if (bv + bi > 0) {
         mbar_arrive_expect_tx(my_bar + s, bv + bi);
-        if (bi) bulk_g2s(st_base, (FMT == 0) ? (const void*)(idx + e) : (const void*)(cidx + c0), bi, my_bar + s, policy);
+        if (bi) bulk_g2s(st_base, (FMT == 0) ? (const void*)(idx + e) : (const void*)csrc, bi, my_bar + s, policy);
         if (bv) bulk_g2s(st_base + SM::kIdx, val + e, bv, my_bar + s, policy);
       } else {
         mbar_arrive(my_bar + s);
@@ -637,26 +647,27 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
 #pragma unroll
         for (int u = 0; u < 8; ++u) cc[u] = si[32 * u];
       } else {
-        // run-compressed index (compress.cuh): H = head bits of the step; my run's head is the last head at or
-        // below my lane: index = heads[heads before the step + popc(H & lanes <= mine) - 1] + lane
+        // run-compressed index (compress.cuh): H = head bits of the step; my run's head is the last head at or below
+        // my lane: index = heads[heads before the step + popc(H & lanes <= mine) - 1] - 32 + lane (the heads are
+        // stored biased by 32 - position, the lane's part of the sum sits in the gather base xl)
         const uint32_t* hw = reinterpret_cast<const uint32_t*>(sb) + rr * 8;
-        const int32_t* heads = reinterpret_cast<const int32_t*>(sb + TILE / 8) - 1;
+        const uint32_t* hp = reinterpret_cast<const uint32_t*>(sb + TILE / 8) - 1;  // -1: popc counts my own head
         const uint32_t le = 0xffffffffu >> (31 - lane);
-        int hb = 0;  // heads in the earlier steps of the tile
-        for (int q = 0; q < rr * 8; ++q) hb += __popc(hw[q - rr * 8]);
+        for (int q = 0; q < rr * 8; ++q) hp += __popc(hw[q - rr * 8]);  // heads in the earlier rounds of the tile
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
           const uint32_t H = hw[u];
-          cc[u] = (uint32_t)(heads[hb + __popc(H & le)] + lane);
-          hb += __popc(H);
+          cc[u] = hp[__popc(H & le)];
+          hp += __popc(H);
         }
       }
+      const double* xg = (FMT == 0) ? x : x + lane - 32;  // FMT 1: biased heads
       if (full) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) xx[u] = __ldg(x + cc[u]);
+        for (int u = 0; u < 8; ++u) xx[u] = __ldg(xg + cc[u]);
       } else {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) xx[u] = (pos0 + 32 * u + lane < cx.len) ? __ldg(x + cc[u]) : 0.0;
+        for (int u = 0; u < 8; ++u) xx[u] = (pos0 + 32 * u + lane < cx.len) ? __ldg(xg + cc[u]) : 0.0;
       }
     };
     // round r with its gathers in xc; the gathers of round r + 1 go to xn meanwhile

@@ -401,12 +401,19 @@ def test_update_values_equals_create_from_scratch(tl, cfg0):
     m, n, rp, ci, va = cfg0["m"], cfg0["n"], cfg0["rp"], cfg0["ci"], cfg0["va"]
     b, damp = cfg0["b"], cfg0["damp"]
     S = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va))
+    S.solve(dev(b), damp, 0.0, 0.0, 12)  # a graph is captured with the old value pointer: the refresh must not replay it
+    S.solve_multi(torch.stack([dev(b), dev(b)], dim=1).contiguous(), damp, 0.0, 0.0, 12)
     va2 = va * (1.0 + 0.2 * rng.standard_normal(len(va)))
     S.update_values(dev(va2))
+    torch.cuda.empty_cache()
+    junk = torch.full((len(va),), float("nan"), dtype=torch.float64, device="cuda")  # likely reuses the freed old array
     cp, ri, cv = (t.cpu().numpy() for t in S.csc())
     ocp, ori, ocv = oracle.csr_to_csc(m, n, rp, ci, va2)
     assert np.array_equal(cp, ocp) and np.array_equal(ri, ori) and np.array_equal(cv, ocv)
     fresh = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va2))
+    Xm, _ = S.solve_multi(torch.stack([dev(b), dev(b)], dim=1).contiguous(), damp, 0.0, 0.0, 12)
+    Xf, _ = fresh.solve_multi(torch.stack([dev(b), dev(b)], dim=1).contiguous(), damp, 0.0, 0.0, 12)
+    assert torch.equal(Xm, Xf)
     for acc in (1, 0):
         for cz in (0, 1):
             S.set(accumulate=acc, compress=cz)
