@@ -336,11 +336,13 @@ tomo_status_t build_csc(tomo_lsqr_s* h, cudaStream_t st, bool only_pos) {
   int64_t T = std::min<int64_t>((int64_t)h->sms * 16, std::max<int64_t>(32, (int64_t)(4.0e9 / (4.0 * (double)n))));
   T = std::max<int64_t>(1, std::min<int64_t>(T, m));
   int32_t* chunk = nullptr; uint32_t* cnt = nullptr; int64_t* coltotal = nullptr;
-  CK(cudaMalloc(&chunk, sizeof(int32_t) * (T + 1)));
-  cudaError_t e = cudaMalloc(&cnt, sizeof(uint32_t) * T * n);
-  if (e != cudaSuccess) { cudaFree(chunk); return cuda_fail(e, "cudaMalloc(transpose scratch)"); }
+  auto drop_pos = [&]() { if (only_pos) { cudaFree(h->pos); h->pos = nullptr; } };  // a half-built permutation must not survive
+  cudaError_t e = cudaMalloc(&chunk, sizeof(int32_t) * (T + 1));
+  if (e != cudaSuccess) { drop_pos(); return cuda_fail(e, "cudaMalloc(transpose chunks)"); }
+  e = cudaMalloc(&cnt, sizeof(uint32_t) * T * n);
+  if (e != cudaSuccess) { cudaFree(chunk); drop_pos(); return cuda_fail(e, "cudaMalloc(transpose scratch)"); }
   e = cudaMalloc(&coltotal, sizeof(int64_t) * n);
-  if (e != cudaSuccess) { cudaFree(chunk); cudaFree(cnt); return cuda_fail(e, "cudaMalloc(coltotal)"); }
+  if (e != cudaSuccess) { cudaFree(chunk); cudaFree(cnt); drop_pos(); return cuda_fail(e, "cudaMalloc(coltotal)"); }
   h->scratch_bytes = (double)(sizeof(uint32_t) * T * n + sizeof(int64_t) * n + sizeof(int32_t) * (T + 1));
   tomo_status_t rc = TOMO_OK;
   cudaEvent_t k0 = nullptr, k1 = nullptr;

@@ -64,7 +64,10 @@ struct CtaRec {        // what a warp (shared memory) or a CTA (global memory) l
 };
 
 constexpr int kBig = 0x3fffffff;  // "beyond the range" for relative element offsets
-constexpr int kPendRows = 4;      // finished rows whose per-lane partials wait in shared memory for one common reduction
+#ifndef TOMO_PEND
+#define TOMO_PEND 4
+#endif
+constexpr int kPendRows = TOMO_PEND;  // finished rows whose per-lane partials wait in shared memory for one common reduction (1, 2, 4 or 8)
 
 template <typename CFG, typename VT, int FMT>
 struct WSmem {
@@ -290,21 +293,22 @@ __device__ __forceinline__ void win_advance(ST& st, const WCtx& cx) {
 }
 __device__ __forceinline__ int64_t row_number(const WCtx& cx, int k) { return cx.rid ? (int64_t)cx.rid[k] : (int64_t)k; }
 
-// The rows that ended since the last flush: their per-lane partials sit in shared memory, [slot][lane].  Eight lanes per
-// row add four partials each (lane q takes lanes q, q+8, q+16, q+24: conflict-free), three butterfly steps close the
-// sum, the first lane of each group finishes its row.  One reduction for kPendRows rows instead of one (5 shuffle
+// The rows that ended since the last flush: their per-lane partials sit in shared memory, [slot][lane].  32 / kPendRows
+// lanes per row add kPendRows partials each (with 4 rows: lane q takes lanes q, q+8, q+16, q+24: conflict-free), a
+// butterfly closes the sum, the first lane of each group finishes its row.  One reduction for kPendRows rows instead of one (5 shuffle
 // steps + the finish code in ONE lane) per row.
 template <int MODE, int OP>
 __device__ __forceinline__ void flush_rows(WSweep<MODE>& st, const WCtx& cx) {
   const int lane = threadIdx.x & 31;
   __syncwarp();
-  const int k = lane >> 3, q = lane & 7;
+  constexpr int LPR = 32 / kPendRows;  // lanes per row
+  const int k = lane / LPR, q = lane % LPR;
   const double2* p = cx.pend + k * 32 + q;
   Acc<MODE> a = acc_of<MODE>(p[0]);
 #pragma unroll
-  for (int i = 1; i < 4; ++i) a.merge(acc_of<MODE>(p[8 * i]));
+  for (int i = 1; i < kPendRows; ++i) a.merge(acc_of<MODE>(p[LPR * i]));
 #pragma unroll
-  for (int off = 1; off < 8; off <<= 1) {
+  for (int off = 1; off < LPR; off <<= 1) {
     double2 o = a.pack();
     o.x = __shfl_xor_sync(0xffffffffu, o.x, off);
     o.y = __shfl_xor_sync(0xffffffffu, o.y, off);
