@@ -691,14 +691,40 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
       if (rr == RPT - 1 && t + NS < ntiles) issue_tile(t + NS, true);  // the tile is in registers: its stage is refilled
       consume_round<MODE, OP, SCALE_X>(st, cx, vv, xc, pos0, sx);
     };
+    // a full round that lies inside the open row (P0), straight-line: gathers of the next round, values, refill, mac8
+    auto straight = [&](int r, double (&xc)[8], double (&xn)[8]) {
+      gather(r + 1, xn);
+      const int t = r / RPT, rr = r % RPT;
+      const VT* sv = reinterpret_cast<const VT*>(stage_ptr(t % NS) + SM::kIdx) + rr * 256 + lane;
+      double vv[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) vv[u] = (double)sv[32 * u];
+      if (rr == RPT - 1 && t + NS < ntiles) issue_tile(t + NS, true);
+      if (SCALE_X) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) xc[u] = xc[u] * sx;
+      }
+      st.acc.mac8(vv, xc);
+    };
     double xa[8], xb[8];
     gather(0, xa);
+    int r = 0;
 #pragma unroll 1
-    for (int r = 0; r < nr; ++r) {  // ONE copy of the round in the code: unrolling twice to swap the gather register sets, or moving
-                                    // the general shape out of line, measured slower (instruction cache / call overhead)
+    while (r < nr) {
+      // pairs of rounds inside the open row: only the straight-line part exists twice in the code, the two gather
+      // register sets swap roles and nothing is copied
+#pragma unroll 1
+      while (r + 2 < nr && st.next_b > ((r + 2) << 8)) {
+        straight(r, xa, xb);
+        straight(r + 1, xb, xa);
+        r += 2;
+      }
+      // any round (ONE copy of the general code: unrolling all of it twice, or moving the general row shape out of
+      // line, measured slower — instruction cache / call overhead); the gathers move over
       body(r, xa, xb);
 #pragma unroll
       for (int u = 0; u < 8; ++u) xa[u] = xb[u];
+      ++r;
     }
     rec.head = st.h_val; rec.head_state = st.h_state;
   }
