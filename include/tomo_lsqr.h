@@ -19,7 +19,7 @@
  *          rejected with TOMO_ERR_NOT_DEVICE_PTR.  h_* and `res`, `out`: HOST pointers.
  *   CSR  : rowptr int64[m+1] (rowptr[0]=0, rowptr[m]=nnz, non-decreasing), colind int32[nnz] with
  *          0 <= col < n STRICTLY INCREASING inside each row (sorted, no duplicates), vals fp64[nnz] or
- *          fp32[nnz], all finite.  1 <= m, n < 2^31, 0 <= nnz < 2^62.  colind and vals must be 16-byte
+ *          fp32[nnz], all finite.  1 <= m, n < 2^31, 0 <= nnz < 2^40.  colind and vals must be 16-byte
  *          aligned.  Violations -> TOMO_ERR_BAD_CSR / TOMO_ERR_INVALID_ARG.
  *   Ownership: the three CSR arrays are BORROWED: the caller keeps them alive and unmodified until
  *          tomo_lsqr_destroy.  The handle owns the CSC copy, the work vectors, the scalars, the graphs.

@@ -410,7 +410,7 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
   *out = nullptr;
   if (vt != TOMO_VAL_F64 && vt != TOMO_VAL_F32) return TOMO_ERR_INVALID_ARG;
   if (m < 1 || n < 1 || nnz < 0) return TOMO_ERR_INVALID_ARG;
-  if (m >= (int64_t)INT32_MAX || n >= (int64_t)INT32_MAX || nnz >= ((int64_t)1 << 62)) return TOMO_ERR_RANGE;
+  if (m >= (int64_t)INT32_MAX || n >= (int64_t)INT32_MAX || nnz >= ((int64_t)1 << 40)) return TOMO_ERR_RANGE;  // warp ranges hold 32-bit relative offsets
   if (!d_rowptr || (nnz > 0 && (!d_colind || !d_vals))) return TOMO_ERR_INVALID_ARG;
   int dev = 0, major = 0, sms = 0;
   CK(cudaGetDevice(&dev));

@@ -15,11 +15,12 @@
 //     to registers and all eight gathers of x are issued at once; the gathers of round r+1 are in flight
 //     while round r is multiplied and summed (two register sets), which hides the L2 latency of the gather; the
 //     values are read from the ring when the round is summed.
-//   * The per-lane accumulator of the open row lives across rounds and tiles; a warp reduction happens once
-//     per row, where the row ends.  A round that lies inside one row is eight exact products and a TwoSum
-//     tree (`mac8`); a round with a row end goes step by step; a step with several row ends (short rows:
-//     the 4-7-entry smoothing rows) uses a segmented warp reduction whose cost does not depend on the
-//     number of rows in the step.  Row starts come from a 64-entry register window of the row pointers
+//   * The per-lane accumulator of the open row lives across rounds and tiles.  A round that lies inside one row
+//     is eight exact products and a TwoSum tree (`mac8`); pairs of such rounds run a straight-line copy of the
+//     round in which the two gather register sets swap roles.  Where a row ends, its 32 per-lane partials are
+//     parked in shared memory and every fourth row end one common reduction closes four rows (close_row /
+//     flush_rows).  A step with several row ends (short rows: the 4-7-entry smoothing rows) uses a segmented
+//     warp reduction whose cost does not depend on the number of rows in the step.  Row starts come from a 64-entry register window of the row pointers
 //     (two registers per lane, refilled 32 rows at a time, one refill ahead).
 //   * The two rows a warp range may cut (the one open at its start, the one open at its end) leave one
 //     record per warp; warp 0 chains the W records of the CTA with a log-step scan over "carry maps" (fixed
