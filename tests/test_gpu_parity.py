@@ -177,6 +177,58 @@ def test_spmv_random_structures(tl):
         g.S.close()
 
 
+def test_random_structures_all_paths(tl):
+    """24 random row-length mixes (tiny rows, geometric long rows, 10 % long among short, lengths on step / round / tile
+    boundaries, long + smoothing-like halves, one giant row) through every product path: dd SpMV both directions, three
+    LSQR iterations, the compressed index, column 0 of the block solve and the row-sharded solve in 3 blocks — all
+    bitwise the dd oracle; fast-mode SpMV <= 1e-12.  (160 further cases of the same generator were run once by hand.)"""
+    rng = np.random.default_rng(2025)
+    for case in range(24):
+        kind = case % 6
+        m = int(rng.integers(1, 5000))
+        if kind == 0:
+            lens = rng.integers(0, 12, size=m)
+        elif kind == 1:
+            lens = rng.geometric(1.0 / rng.integers(50, 3000), size=m)
+        elif kind == 2:
+            lens = np.where(rng.random(m) < 0.1, rng.integers(200, 4000, size=m), rng.integers(0, 9, size=m))
+        elif kind == 3:
+            lens = rng.choice([0, 1, 31, 32, 33, 255, 256, 257, 511, 512, 513, 1024], size=m)
+        elif kind == 4:
+            lens = np.concatenate([rng.integers(300, 1500, size=m // 2 + 1), rng.integers(4, 8, size=m // 2)])
+        else:
+            lens = rng.integers(0, 5, size=m)
+            lens[rng.integers(0, m)] = int(rng.integers(10000, 400000))
+        lens = np.asarray(lens, dtype=np.int64)
+        m = len(lens)
+        n = int(max(lens.max(), 1) + rng.integers(0, 20000))
+        rp, ci, va = tomogen.random_csr(m, n, np.minimum(lens, n), seed=int(rng.integers(1 << 30)))
+        S = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va))
+        xv, uv, b = rng.standard_normal(n), rng.standard_normal(m), rng.standard_normal(m)
+        o = oracle.lsqr(m, n, rp, ci, va, b, damp=0.3, max_iters=3, mode=oracle.DD)
+        oy, oyt = oracle.spmv(m, n, rp, ci, va, xv, 1), oracle.spmv_t(m, n, rp, ci, va, uv, 1)
+        for cz in (0, 1):
+            S.set(accumulate=1, compress=cz)
+            assert np.array_equal(S.spmv(dev(xv)).cpu().numpy(), oy), (case, cz)
+            assert np.array_equal(S.spmv(dev(uv), transpose=True).cpu().numpy(), oyt), (case, cz)
+            x, res = S.solve(dev(b), 0.3, 0.0, 0.0, 3)
+            assert res.itn == o.itn and np.array_equal(x.cpu().numpy(), o.x), (case, cz)
+            S.set(accumulate=0)
+            assert rel(S.spmv(dev(xv)).cpu().numpy(), oracle.spmv(m, n, rp, ci, va, xv, 0)) <= TOL_SPMV
+        S.set(accumulate=1, compress=0)
+        X, _ = S.solve_multi(dev(np.stack([b, -b, 0.5 * b], axis=1)), 0.3, 0.0, 0.0, 3)
+        assert np.array_equal(X[:, 0].cpu().numpy(), o.x), case
+        if m >= 3:
+            cuts = [0, m // 3, 2 * m // 3, m]
+            blocks = _row_blocks(tl, m, n, rp, ci, va, cuts)
+            xs = torch.empty(n, dtype=torch.float64, device="cuda")
+            tl.tomo_lsqr_solve_sharded([B.h for B in blocks], [dev(b[a:c]) for a, c in zip(cuts[:-1], cuts[1:])], 0.3, 0.0, 0.0, 3, xs)
+            assert np.array_equal(xs.cpu().numpy(), o.x), case
+            for B in blocks:
+                B.close()
+        S.close()
+
+
 def test_spmv_single_row_and_single_column(tl):
     rp, ci, va = tomogen.random_csr(1, 5000, [3000], seed=8)
     check_spmv(Sys(tl, 1, 5000, rp, ci, va), 9)
