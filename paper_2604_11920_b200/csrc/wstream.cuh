@@ -715,7 +715,7 @@ k_wstream(const int64_t* __restrict__ ptr, const int32_t* __restrict__ rid, cons
       // pairs of rounds inside the open row: only the straight-line part exists twice in the code, the two gather
       // register sets swap roles and nothing is copied
 #pragma unroll 1
-      while (r + 2 < nr && st.next_b > ((r + 2) << 8)) {
+      while (FMT == 0 && r + 2 < nr && st.next_b > ((r + 2) << 8)) {  // (FMT 1: the decode makes the copy too large for the instruction cache)
         straight(r, xa, xb);
         straight(r + 1, xb, xa);
         r += 2;
