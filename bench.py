@@ -137,6 +137,24 @@ def workload_name(s) -> str:
             f"atol=btol={s.solve['atol']:g}, max_iters {s.solve['max_iters']}")
 
 
+def workload_config(s, args, iterations_per_step: int, world: int = 1) -> dict:
+    """The `config` object of a bench line: names the workload and how the GPU arm is run on it.  Both arms print the
+    SAME object for the same arguments (the reference arm times a bounded sample of this workload; its `cpu_baseline.sample`
+    says which)."""
+    m, n, nnz, nrhs = s.dims.m, s.dims.n, s.dims.nnz, s.dims.nrhs
+    vbytes = 4 if args.vals == "f32" else 8
+    ab = algorithmic_bytes(m, n, nnz, vbytes) if nrhs == 1 else block_bytes(m, n, nnz, nrhs, vbytes)
+    return {"workload": workload_name(s), "iterations_per_step": iterations_per_step,
+            "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
+            "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
+            "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
+            "index": "run-compressed (compress=1)" if args.compress else "int32 per nonzero",
+            "parallelism": "replicas" if world > 1 else "single GPU",
+            "l2": (f"inputs larger than L2: {ab['iteration'] / 1e9:.2f} GB streamed per iteration vs 126 MB L2, no flush needed"
+                   if ab["iteration"] > 2 * 126e6 else
+                   f"working set {ab['iteration'] / 1e6:.1f} MB per iteration fits in L2: launch-latency-bound workload, no roofline claim")}
+
+
 def ref_iters_for(args) -> int:
     """Oracle iterations per timed sample: about 10-30 s of CPU work (config 2 is 19 x config 1)."""
     return args.ref_iters if args.config != 2 else max(1, args.ref_iters // 10)
@@ -172,12 +190,13 @@ def run_reference(args) -> dict:
         assert r.itn == iters
     total = sum(times)
     value = iters * args.steps / total
-    sample = f"{iters} iterations (plus the init pass) of the full configs[{args.config}] system per step"
+    sample = (f"{iters} iterations (plus the init pass) of the full configs[{args.config}] system per step, oracle in plain fp64 mode, "
+              f"first right-hand side; the GPU arm runs the whole workload named in config")
     return {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(s), "l2": "per-iteration working set 4.7 GB >> L2"},
+        "config": workload_config(s, args, int(s.solve["max_iters"]) * int(s.dims.nrhs), max(1, args.gpus)),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -454,13 +473,7 @@ def run_ours(args) -> dict | None:
         "metric": METRIC, "value": its / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": workload_name(s), "iterations_per_step": its // max(1, args.steps * world),
-                   "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
-                   "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
-                   "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
-                   "index": "run-compressed (compress=1)" if args.compress else "int32 per nonzero",
-                   "parallelism": "replicas" if world > 1 else "single GPU",
-                   "l2": f"inputs larger than L2: {ab['iteration'] / 1e9:.2f} GB streamed per iteration vs 126 MB L2, no flush needed"},
+        "config": workload_config(s, args, its // max(1, args.steps * world), world),
         "effective_gbs": eff,
         "create_ms": r["create_ms"], "transpose_ms": r["transpose_ms"], "create_wall_ms": r["create_wall_ms"],
         "create_note": "create_ms / transpose_ms: CUDA events inside tomo_lsqr_create (kernels + its cudaMalloc calls); create_wall_ms: host clock around the call",
