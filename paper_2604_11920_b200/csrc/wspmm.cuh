@@ -143,6 +143,11 @@ __device__ __forceinline__ void consume_round8(MSweep<MODE>& st, const WCtx& cx,
     x1[u] = SCALE_X ? xx[u].y * sx1 : xx[u].y;
   }
   if (st.next_b > pos0 + 64) {  // the round lies inside the open row (lanes behind the range hold zeros)
+    if (MODE == 1) {  // dd: two interleaved chains of plain mac()s; the TwoSum tree of mac8 costs registers here (measured +10 %)
+#pragma unroll
+      for (int u = 0; u < 8; ++u) { st.a0.mac(vv[u], x0[u]); st.a1.mac(vv[u], x1[u]); }
+      return;
+    }
     st.a0.mac8(vv, x0);
     st.a1.mac8(vv, x1);
     return;
