@@ -53,7 +53,8 @@ typedef enum {
   TOMO_ERR_OOM = 4,
   TOMO_ERR_CUDA = 5,
   TOMO_ERR_UNSUPPORTED_ARCH = 6,
-  TOMO_ERR_RANGE = 7
+  TOMO_ERR_RANGE = 7,
+  TOMO_ERR_NOALLOC_LIMIT = 8   /* tomo_lsqr_spmv_noalloc: the matrix or the device is beyond the static scratch array */
 } tomo_status_t;
 
 typedef enum { TOMO_VAL_F64 = 0, TOMO_VAL_F32 = 1 } tomo_valtype_t;
@@ -185,6 +186,33 @@ tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value
  * replayed graphs included); "cta_busy_min" / "cta_busy_mean" / "cta_busy_max": busy cycles of the persistent
  * CTAs in the most recent sparse-product launch (load balance of the static split). */
 tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, double* out);
+
+/* The sparse product for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): d_y <- A d_x over the caller's CSR with the streaming kernel of the solver
+ * (k_wstream, the "sparse matrix-vector multiplications" PAPER.md P:144 offloads), WITHOUT a handle and without
+ * any cudaMalloc / cudaFree / allocating library call.  Everything tomo_lsqr_create would allocate for this
+ * product (the warp split points, the per-CTA records and tickets of the kernel, and, when the matrix has rows
+ * without entries, the compacted row pointers and the row lists) lives in ONE file-scope static __device__ array
+ * of TOMO_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.
+ *   m, n, nnz, d_rowptr int64[m+1], d_colind int32[nnz], d_vals (fp64 or fp32 per vt): DEVICE arrays as for
+ *     tomo_lsqr_create (same alignment rules).  They are NOT validated here: pass arrays tomo_lsqr_create accepts.
+ *   accumulate: 0 = fp64 FMA sums, 1 = double-double sums rounded once (as option "accumulate").
+ *   d_x fp64[n] in, d_y fp64[m] out (every entry is written), both DEVICE, caller-owned.
+ * Limits: m <= TOMO_NOALLOC_MAX_ROWS and a device with at most TOMO_NOALLOC_MAX_SMS multiprocessors, otherwise
+ *   TOMO_ERR_NOALLOC_LIMIT and nothing is launched; m, n, nnz ranges as for create (TOMO_ERR_RANGE).
+ * Results: the same kernel, split points and summation order as tomo_lsqr_spmv(h, 0, ...) on a handle with
+ *   default options, so the output is bitwise that of the handle path in both accumulation modes.
+ * Sharing: every call on a device uses the same array, which keeps the previous call's contents; the call clears
+ *   what must start at zero (the ticket words and the empty-row counter) itself.  Calls that overlap on the GPU
+ *   (two streams, two host threads) RACE on the array: serialise them.  The call synchronises `cuda_stream` twice
+ *   (it reads the number of rows without entries back to the host, and waits for the product before returning).
+ * Errors: INVALID_ARG, NOT_DEVICE_PTR, RANGE, NOALLOC_LIMIT, UNSUPPORTED_ARCH, CUDA. */
+#define TOMO_NOALLOC_MAX_ROWS 524288
+#define TOMO_NOALLOC_MAX_SMS 256
+#define TOMO_NOALLOC_SCRATCH_BYTES (24 * (TOMO_NOALLOC_MAX_ROWS + 64) + 131072)   /* 12.1 MiB */
+tomo_status_t tomo_lsqr_spmv_noalloc(int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr, const int32_t* d_colind,
+                                const void* d_vals, tomo_valtype_t vt, int accumulate, const double* d_x, double* d_y,
+                                void* cuda_stream);
 
 void tomo_lsqr_destroy(tomo_lsqr_t h);
 

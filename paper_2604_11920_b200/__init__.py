@@ -17,14 +17,15 @@ LIB_PATH = os.path.join(_HERE, "libtomolsqr.so")
 
 TOMO_OK = 0
 TOMO_ERR_INVALID_ARG, TOMO_ERR_BAD_CSR, TOMO_ERR_NOT_DEVICE_PTR, TOMO_ERR_OOM = 1, 2, 3, 4
-TOMO_ERR_CUDA, TOMO_ERR_UNSUPPORTED_ARCH, TOMO_ERR_RANGE = 5, 6, 7
+TOMO_ERR_CUDA, TOMO_ERR_UNSUPPORTED_ARCH, TOMO_ERR_RANGE, TOMO_ERR_NOALLOC_LIMIT = 5, 6, 7, 8
+TOMO_NOALLOC_MAX_ROWS, TOMO_NOALLOC_MAX_SMS = 524288, 256   # include/tomo_lsqr.h
 TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
     "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
     "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values", "tomo_lsqr_solve_sharded",
-    "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_destroy", "tomo_status_string",
+    "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_spmv_noalloc", "tomo_lsqr_destroy", "tomo_status_string",
 )
 
 
@@ -71,6 +72,7 @@ def load() -> ctypes.CDLL:
     lib.tomo_lsqr_get_csc.argtypes = [vp, vp, vp, vp, vp]
     lib.tomo_lsqr_set_option.argtypes = [vp, ctypes.c_char_p, i64]
     lib.tomo_lsqr_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(f64)]
+    lib.tomo_lsqr_spmv_noalloc.argtypes = [i64, i64, i64, vp, vp, vp, ci, ci, vp, vp, vp]
     lib.tomo_lsqr_destroy.argtypes = [vp]
     lib.tomo_lsqr_destroy.restype = None
     lib.tomo_status_string.argtypes = [ci]
@@ -171,6 +173,14 @@ def tomo_lsqr_spmv(h, transpose, d_in, d_out, stream=None) -> None:
     st = load().tomo_lsqr_spmv(h, int(transpose), _ptr(d_in), _ptr(d_out), _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_spmv")
+
+
+def tomo_lsqr_spmv_noalloc(m, n, nnz, d_rowptr, d_colind, d_vals, vt, accumulate, d_x, d_y, stream=None) -> None:
+    """d_y <- A d_x over the caller's CSR without a handle and without any allocation (static scratch array in the library)."""
+    st = load().tomo_lsqr_spmv_noalloc(int(m), int(n), int(nnz), _ptr(d_rowptr), _ptr(d_colind), _ptr(d_vals), int(vt), int(accumulate),
+                                  _ptr(d_x), _ptr(d_y), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_spmv_noalloc")
 
 
 class _RawBytes:

@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -26,6 +27,7 @@ using namespace tomo;
 namespace {
 
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+thread_local char g_noalloc_msg[256] = "tomo_lsqr_spmv_noalloc: beyond the static scratch array (TOMO_NOALLOC_MAX_ROWS / TOMO_NOALLOC_MAX_SMS)";
 
 tomo_status_t cuda_fail(cudaError_t e, const char* what) {
   snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error in %s: %s", what, cudaGetErrorString(e));
@@ -1187,6 +1189,130 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   return TOMO_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// tomo_lsqr_spmv_noalloc: the plain product over the caller's CSR for callers that cannot allocate.  The scratch of the
+// streaming kernel (and of the compaction of rows without entries) lives in one file-scope device array.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+// layout of the static scratch array; every member starts at a multiple of 256 bytes
+struct NoAllocScratch {
+  alignas(256) unsigned char sc[4096];                                          // Scalars (only the ticket words are used)
+  alignas(256) int cnt[64];                                                     // number of rows without entries
+  alignas(256) CtaRec rec[TOMO_NOALLOC_MAX_SMS];                                // one record per persistent CTA
+  alignas(256) double2 part[TOMO_NOALLOC_MAX_SMS + 2];                          // per-CTA ||.||^2 partials (unused by the plain product, still written)
+  alignas(256) int64_t wE[TOMO_NOALLOC_MAX_SMS * WC::W + 1];                    // element split points of the warp ranges
+  alignas(256) int32_t wR[TOMO_NOALLOC_MAX_SMS * WC::W + 1];                    // ... and their first rows
+  alignas(256) int64_t pos[TOMO_NOALLOC_MAX_ROWS + 1];                          // exclusive scan of the non-empty flags
+  alignas(256) int64_t cptr[TOMO_NOALLOC_MAX_ROWS + 1];                         // non-empty flags, then the compacted row pointers
+  alignas(256) int32_t rid[TOMO_NOALLOC_MAX_ROWS];                              // row numbers of the non-empty rows
+  alignas(256) int32_t erows[TOMO_NOALLOC_MAX_ROWS];                            // rows without entries
+};
+static_assert(sizeof(Scalars) <= 4096, "Scalars outgrew its slot of the static scratch");
+static_assert(sizeof(NoAllocScratch) <= TOMO_NOALLOC_SCRATCH_BYTES, "TOMO_NOALLOC_SCRATCH_BYTES is too small for the layout");
+
+}  // namespace
+
+// The name below is a HOST-side stand-in in host code, not a device address: the address a kernel can use comes
+// from cudaGetSymbolAddress, once per device, with that device current (noalloc_setup).
+static __device__ __align__(256) unsigned char g_noalloc_scratch[TOMO_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+NoAllocScratch* g_noalloc_ptr[kNoAllocMaxDevices] = {};   // device address of the array on device d (NULL: not set up yet)
+
+// once per device (the device is current): address of the device's copy of the array, shared-memory opt-in of the
+// four instantiations the entry launches
+tomo_status_t noalloc_setup(int dev, NoAllocScratch** out) {
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static scratch)");
+    if (!p || ((uintptr_t)p & 255u)) { snprintf(g_cuda_msg, sizeof(g_cuda_msg), "static scratch: bad device address"); return TOMO_ERR_CUDA; }
+    if ((e = stream_attr_one<WC, 0, double, OP_PLAIN, 0>()) != cudaSuccess || (e = stream_attr_one<WC, 1, double, OP_PLAIN, 0>()) != cudaSuccess ||
+        (e = stream_attr_one<WC, 0, float, OP_PLAIN, 0>()) != cudaSuccess || (e = stream_attr_one<WC, 1, float, OP_PLAIN, 0>()) != cudaSuccess)
+      return cuda_fail(e, "cudaFuncSetAttribute(shared memory opt-in)");
+    g_noalloc_ptr[dev] = static_cast<NoAllocScratch*>(p);
+  }
+  *out = g_noalloc_ptr[dev];
+  return TOMO_OK;
+}
+
+template <int MODE, typename VT>
+cudaError_t noalloc_launch(int sms, const int64_t* ptr, const int32_t* rid, const int32_t* idx, const VT* val, int64_t nnz, int nrows,
+                           const int32_t* erows, int n_empty, const double* x, double* y, NoAllocScratch* S, cudaStream_t st) {
+  k_wstream<WC, MODE, VT, OP_PLAIN, 0><<<sms, WC::THREADS, WSmem<WC, VT, 0>::kTotal, st>>>(
+      ptr, rid, idx, val, nullptr, nullptr, nnz, nrows, erows, n_empty, x, y, S->wE, S->wR, S->rec, reinterpret_cast<Scalars*>(S->sc), S->part);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_spmv_noalloc(int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr, const int32_t* d_colind,
+                                           const void* d_vals, tomo_valtype_t vt, int accumulate, const double* d_x, double* d_y,
+                                           void* cuda_stream) {
+  if (vt != TOMO_VAL_F64 && vt != TOMO_VAL_F32) return TOMO_ERR_INVALID_ARG;
+  if (accumulate != 0 && accumulate != 1) return TOMO_ERR_INVALID_ARG;
+  if (m < 1 || n < 1 || nnz < 0 || !d_x || !d_y) return TOMO_ERR_INVALID_ARG;
+  if (m >= (int64_t)INT32_MAX || n >= (int64_t)INT32_MAX || nnz >= ((int64_t)1 << 40)) return TOMO_ERR_RANGE;
+  if (!d_rowptr || (nnz > 0 && (!d_colind || !d_vals))) return TOMO_ERR_INVALID_ARG;
+  int dev = 0, major = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) return TOMO_ERR_UNSUPPORTED_ARCH;
+  if (m > (int64_t)TOMO_NOALLOC_MAX_ROWS) {
+    snprintf(g_noalloc_msg, sizeof(g_noalloc_msg), "tomo_lsqr_spmv_noalloc: m = %lld rows exceeds TOMO_NOALLOC_MAX_ROWS = %d (the static scratch array); use a handle (tomo_lsqr_create + tomo_lsqr_spmv)",
+             (long long)m, (int)TOMO_NOALLOC_MAX_ROWS);
+    return TOMO_ERR_NOALLOC_LIMIT;
+  }
+  if (sms > TOMO_NOALLOC_MAX_SMS || dev >= kNoAllocMaxDevices) {
+    snprintf(g_noalloc_msg, sizeof(g_noalloc_msg), "tomo_lsqr_spmv_noalloc: device %d with %d multiprocessors is beyond TOMO_NOALLOC_MAX_SMS = %d / %d devices (the static scratch array)",
+             dev, sms, (int)TOMO_NOALLOC_MAX_SMS, kNoAllocMaxDevices);
+    return TOMO_ERR_NOALLOC_LIMIT;
+  }
+  if (!is_device_ptr(d_rowptr) || !is_device_ptr(d_x) || !is_device_ptr(d_y) || (nnz > 0 && (!is_device_ptr(d_colind) || !is_device_ptr(d_vals))))
+    return TOMO_ERR_NOT_DEVICE_PTR;
+  if (((uintptr_t)d_colind & 15u) || ((uintptr_t)d_vals & 15u) || ((uintptr_t)d_rowptr & 7u)) return TOMO_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  NoAllocScratch* S = nullptr;
+  { tomo_status_t rc = noalloc_setup(dev, &S); if (rc != TOMO_OK) return rc; }
+
+  // the array keeps the last call's contents: the ticket words and the counter must start at zero
+  CK(cudaMemsetAsync(S->sc, 0, sizeof(Scalars), st));
+  CK(cudaMemsetAsync(S->cnt, 0, sizeof(int), st));
+  k_count_empty<<<sms * 4, 256, 0, st>>>(d_rowptr, m, S->cnt);
+  CK(cudaGetLastError());
+  int cnt = 0;
+  CK(cudaMemcpyAsync(&cnt, S->cnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const int64_t* ptr = d_rowptr; const int32_t* rid = nullptr; const int32_t* erows = nullptr;
+  int nrows = (int)m;
+  if (cnt > 0) {  // rows without entries never enter the stream (build_dir): compact them away, into the static array
+    k_flag_nonempty<<<sms * 4, 256, 0, st>>>(d_rowptr, m, S->cptr);
+    k_exscan<<<1, 1024, 0, st>>>(S->cptr, m, S->pos);
+    k_compact_rows<<<sms * 4, 256, 0, st>>>(d_rowptr, m, S->pos, S->cptr, S->rid, S->erows);
+    CK(cudaGetLastError());
+    ptr = S->cptr; rid = S->rid; erows = S->erows; nrows = (int)(m - cnt);
+  }
+  const int parts = sms * WC::W;  // the split a handle with default options uses (row_cost 320): same summation order
+  k_stream_partition<<<(parts + 1 + 127) / 128, 128, 0, st>>>(ptr, nrows, nnz, parts, 320, WC::TILE, S->wE, S->wR);
+  CK(cudaGetLastError());
+  cudaError_t e;
+  if (vt == TOMO_VAL_F64)
+    e = accumulate ? noalloc_launch<1, double>(sms, ptr, rid, d_colind, (const double*)d_vals, nnz, nrows, erows, cnt, d_x, d_y, S, st)
+                   : noalloc_launch<0, double>(sms, ptr, rid, d_colind, (const double*)d_vals, nnz, nrows, erows, cnt, d_x, d_y, S, st);
+  else
+    e = accumulate ? noalloc_launch<1, float>(sms, ptr, rid, d_colind, (const float*)d_vals, nnz, nrows, erows, cnt, d_x, d_y, S, st)
+                   : noalloc_launch<0, float>(sms, ptr, rid, d_colind, (const float*)d_vals, nnz, nrows, erows, cnt, d_x, d_y, S, st);
+  if (e != cudaSuccess) return cuda_fail(e, "k_wstream (no-alloc product)");
+  CK(cudaStreamSynchronize(st));
+  return TOMO_OK;
+}
+
 extern "C" const char* tomo_status_string(tomo_status_t s) {
   switch (s) {
     case TOMO_OK: return "ok";
@@ -1197,6 +1323,7 @@ extern "C" const char* tomo_status_string(tomo_status_t s) {
     case TOMO_ERR_CUDA: return g_cuda_msg;
     case TOMO_ERR_UNSUPPORTED_ARCH: return "device is not compute capability 10.x (sm_100a build, no fallback)";
     case TOMO_ERR_RANGE: return "m, n or nnz out of range";
+    case TOMO_ERR_NOALLOC_LIMIT: return g_noalloc_msg;
   }
   return "unknown status";
 }
