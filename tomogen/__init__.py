@@ -54,6 +54,12 @@ def _load():
             getattr(lib, name).restype = None
         lib.tomogen_fill.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         lib.tomogen_fill.restype = None
+        lib.tomogen_lateral_ptr.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.tomogen_lateral_ptr.restype = None
+        lib.tomogen_lateral_fill.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.tomogen_lateral_fill.restype = None
+        lib.tomogen_kernels.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.tomogen_kernels.restype = None
         for name in ("tomogen_xtrue", "tomogen_rhs"):
             getattr(lib, name).argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
             getattr(lib, name).restype = None
@@ -161,6 +167,34 @@ class System:
             va_d[e0:e1] = torch.from_numpy(va).cuda()
         return torch.from_numpy(rp).cuda(), ci_d, va_d
 
+    # --- the same matrix in factored form (Eq. 5: lateral footprint x depth kernel) --------------
+    def factored(self):
+        """The parts tomogen multiplies out into the CSR values: a dict with
+        npairs, nper, nnodes, nz, klen; lptr int64[npairs+1], lnode int32[E], lw float64[E] (the pairs' lateral
+        footprints W, nodes ascending); kj0 int32[nper], kern float64[nper, klen] (depth-kernel windows);
+        sptr/sidx/svals: the smoothing rows as a CSR block of their own (ms = n rows).
+        Row q*nper + p of the data block has value lw[e] * kern[p, t] at column lnode[e]*nz + kj0[p] + t."""
+        d = self.dims
+        lib = _load()
+        lptr = np.empty(d.npairs + 1, dtype=np.int64)
+        lib.tomogen_lateral_ptr(self._h, _p(lptr))
+        E = int(lptr[-1])
+        lnode = np.empty(E, dtype=np.int32)
+        lw = np.empty(E, dtype=np.float64)
+        lib.tomogen_lateral_fill(self._h, 0, d.npairs, _p(lptr), _p(lnode), _p(lw))
+        kj0 = np.empty(d.nper, dtype=np.int32)
+        kern = np.empty((d.nper, d.keep), dtype=np.float64)
+        lib.tomogen_kernels(self._h, _p(kj0), _p(kern))
+        rp = self.rowptr()
+        s0 = int(rp[d.m_data])
+        sptr = (rp[d.m_data:] - s0).astype(np.int64)
+        snnz = int(sptr[-1])
+        sidx = np.empty(snnz, dtype=np.int32)
+        svals = np.empty(snnz, dtype=np.float64)
+        self.fill(d.m_data, d.m, sidx, svals)
+        return dict(npairs=d.npairs, nper=d.nper, nnodes=d.nx * d.ny, nz=d.nz, klen=d.keep, lptr=lptr, lnode=lnode, lw=lw,
+                    kj0=kj0, kern=kern, sptr=sptr, sidx=sidx, svals=svals)
+
     # --- vectors ----------------------------------------------------------------------------
     def x_true(self, rhs: int = 0) -> np.ndarray:
         x = np.empty(self.dims.n, dtype=np.float64)
@@ -215,3 +249,33 @@ def random_csr(m: int, n: int, row_lengths, seed: int, dtype=np.float64):
     va = rng.standard_normal(rp[-1]).astype(dtype)
     va[va == 0] = 1.0
     return rp, ci, va
+
+
+def random_factored(npairs, nper, nnodes, nz, klen, seed, ms=None, empty_pairs=0.1, empty_nodes=0.1, max_entries=40):
+    """Unstructured factored system (unit tests: odd shapes, empty pairs and nodes, windows at the rim): the dict
+    :meth:`System.factored` returns, with random footprints, windows and a random short-row extra block (ms rows;
+    None: nnodes*nz rows of 0..7 entries; 0: no extra block)."""
+    rng = np.random.default_rng(seed)
+    live = np.flatnonzero(rng.random(nnodes) >= empty_nodes)
+    if len(live) == 0:
+        live = np.array([0])
+    cnt = rng.integers(1, min(max_entries, len(live)) + 1, size=npairs)
+    cnt[rng.random(npairs) < empty_pairs] = 0
+    lptr = np.zeros(npairs + 1, dtype=np.int64)
+    np.cumsum(cnt, out=lptr[1:])
+    lnode = np.empty(int(lptr[-1]), dtype=np.int32)
+    for q in range(npairs):
+        lnode[lptr[q]:lptr[q + 1]] = np.sort(rng.choice(live, size=int(cnt[q]), replace=False))
+    lw = rng.standard_normal(int(lptr[-1]))
+    lw[lw == 0] = 1.0
+    kj0 = rng.integers(0, nz - klen + 1, size=nper).astype(np.int32)
+    kern = rng.standard_normal((nper, klen))
+    n = nnodes * nz
+    if ms is None:
+        ms = n
+    out = dict(npairs=npairs, nper=nper, nnodes=nnodes, nz=nz, klen=klen, lptr=lptr, lnode=lnode, lw=lw, kj0=kj0, kern=kern,
+               sptr=None, sidx=None, svals=None)
+    if ms:
+        sp_, si_, sv_ = random_csr(ms, n, rng.integers(0, min(8, n + 1), size=ms), seed + 1)
+        out.update(sptr=sp_, sidx=si_, svals=sv_)
+    return out

@@ -412,6 +412,39 @@ void tomogen_fill(void* h, int64_t r0, int64_t r1, int32_t* colind, double* vals
   }
 }
 
+// ---- the factored parts of the data block (what tomogen_fill multiplies out): lateral footprints and depth kernels ----
+// lptr[npairs + 1]: offsets of the pairs' lateral node lists
+void tomogen_lateral_ptr(void* h, int64_t* lptr) {
+  Gen* g = (Gen*)h;
+  lptr[0] = 0;
+  for (int64_t p = 0; p < g->npairs; ++p) lptr[p + 1] = lptr[p] + g->pair_nodes[p];
+}
+
+// nodes (ascending inside a pair) and accumulated weights W[k] of pairs [p0, p1), entry e written at e - lptr[p0]
+void tomogen_lateral_fill(void* h, int64_t p0, int64_t p1, const int64_t* lptr, int32_t* node, double* w) {
+  Gen* g = (Gen*)h;
+  const Config& c = g->c;
+  if (p0 < 0) p0 = 0;
+  if (p1 > g->npairs) p1 = g->npairs;
+#pragma omp parallel
+  {
+    Scratch s(c.nx * c.ny);
+#pragma omp for schedule(dynamic, 64)
+    for (int64_t p = p0; p < p1; ++p) {
+      lateral(*g, p, s);
+      int64_t e = lptr[p] - lptr[p0];
+      for (int32_t k : s.touched) { node[e] = k; w[e] = s.W[k]; ++e; }
+    }
+  }
+}
+
+// j0[nper]: first layer of each period's window; kern[nper * keep]: the window values
+void tomogen_kernels(void* h, int32_t* j0, double* kern) {
+  Gen* g = (Gen*)h;
+  std::memcpy(j0, g->kern_j0.data(), sizeof(int32_t) * g->c.nper);
+  std::memcpy(kern, g->kern.data(), sizeof(double) * (size_t)g->c.nper * g->c.keep);
+}
+
 void tomogen_xtrue(void* h, int rhs, double* x) { xtrue(*(Gen*)h, rhs, x); }
 
 void tomogen_raylen(void* h, double* L) { Gen* g = (Gen*)h; std::memcpy(L, g->raylen.data(), sizeof(double) * g->npairs); }
