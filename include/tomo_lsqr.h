@@ -79,6 +79,33 @@ typedef struct {
 tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t nnz, const int64_t* d_rowptr,
                                const int32_t* d_colind, const void* d_vals, tomo_valtype_t vt, void* cuda_stream);
 
+/* NEXT-2, factored form (Eq. 5, unknown ordering Eq. 7): the same solver on
+ *      A = [ A_data ; A_extra ],   A_data[q * nper + p, k * nz + j] = fl( W[q, k] * g_p[j - j0_p] ),  j0_p <= j < j0_p + klen,
+ * without ever storing A_data per nonzero.  q = station pair (ray), p = period, k = lateral node, j = layer:
+ *   W      npairs x nnodes, canonical CSR on the device: d_lptr int64[npairs + 1], d_lnode int32[E] strictly increasing
+ *          inside a pair, d_lw fp64[E] finite (the lateral footprint of the ray; pairs without entries are allowed);
+ *   g      d_kern fp64[nper * klen] (row p = the depth kernel of period p on its window), d_kj0 int32[nper] the first
+ *          layer of each window, 0 <= j0_p and j0_p + klen <= nz;  1 <= nper <= 32, 1 <= klen <= min(nz, 32) (RANGE);
+ *   A_extra  ms x (nnodes * nz) canonical CSR block appended below A_data (the smoothing rows; ms = 0: none):
+ *          d_sptr int64[ms + 1], d_sidx int32[snnz], d_svals fp64[snnz].  Its rows are walked one lane per row.
+ * m = npairs * nper + ms < 2^31, n = nnodes * nz < 2^31.  BORROWED until destroy: d_lptr, d_lnode, d_lw, d_sptr, d_sidx,
+ * d_svals; d_kj0 and d_kern are copied.  The handle owns W by node (CSC), A_extra by column, the static work split.
+ * A lateral entry (12 bytes) stands for nper * klen nonzeros of the CSR form, so the products are bound by fp64
+ * arithmetic instead of HBM (get_info "operator_bytes").  Every product uses the ROUNDED value fl(W g), the number the
+ * CSR form stores: with "accumulate" = 1 all results (tomo_lsqr_spmv, the solves) are bit for bit those of a
+ * tomo_lsqr_create handle on the expanded matrix; with "accumulate" = 0 they agree to rounding (other summation order).
+ * Supported on such a handle: tomo_lsqr_solve / tomo_lsmr_solve, *_solve_host, *_solve_multi (the sides run one after
+ * the other), tomo_lsqr_spmv, the options "check_every", "accumulate", "graph", "profile", "pdl", and get_info.
+ * Not supported (INVALID_ARG): tomo_lsqr_update_values (nothing is stored per nonzero: create again, it costs
+ * milliseconds), tomo_lsqr_get_csc, "compress" = 1, tomo_lsqr_solve_sharded.
+ * Errors: INVALID_ARG, RANGE, NOT_DEVICE_PTR, BAD_CSR (W, A_extra or the kernel table malformed / non-finite),
+ * UNSUPPORTED_ARCH, OOM, CUDA; *out is NULL on error. */
+tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz,
+                                        const int64_t* d_lptr, const int32_t* d_lnode, const double* d_lw, int32_t klen,
+                                        const int32_t* d_kj0, const double* d_kern, int64_t ms, int64_t snnz,
+                                        const int64_t* d_sptr, const int32_t* d_sidx, const double* d_svals,
+                                        void* cuda_stream);
+
 /* NEXT-4: value-only refresh.  The outer Gauss-Newton loop of the inversion
  * re-evaluates G on the same rays and solves again: the sparsity pattern, hence the CSC permutation, the split
  * points and the compressed index, stay; only the values change.  d_vals: device array [nnz] of the handle's value

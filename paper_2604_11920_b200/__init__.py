@@ -23,7 +23,7 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
-    "tomo_lsqr_create", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
+    "tomo_lsqr_create", "tomo_lsqr_create_factored", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
     "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values", "tomo_lsqr_solve_sharded",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_spmv_noalloc", "tomo_lsqr_destroy", "tomo_status_string",
 )
@@ -59,6 +59,7 @@ def load() -> ctypes.CDLL:
     lib = ctypes.CDLL(LIB_PATH)
     vp, i64, i32, f64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int
     lib.tomo_lsqr_create.argtypes = [ctypes.POINTER(vp), i64, i64, i64, vp, vp, vp, ci, vp]
+    lib.tomo_lsqr_create_factored.argtypes = [ctypes.POINTER(vp), i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, vp]
     lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
     lib.tomo_lsmr_solve.argtypes = lib.tomo_lsqr_solve.argtypes
     lib.tomo_lsqr_solve_host.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
@@ -111,6 +112,17 @@ def tomo_lsqr_create(m, n, nnz, d_rowptr, d_colind, d_vals, vt=TOMO_VAL_F64, str
     st = load().tomo_lsqr_create(ctypes.byref(h), m, n, nnz, _ptr(d_rowptr), _ptr(d_colind), _ptr(d_vals), vt, _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_create")
+    return h.value
+
+
+def tomo_lsqr_create_factored(npairs, nper, nnodes, nz, d_lptr, d_lnode, d_lw, klen, d_kj0, d_kern, ms=0, snnz=0,
+                              d_sptr=None, d_sidx=None, d_svals=None, stream=None) -> int:
+    h = ctypes.c_void_p()
+    st = load().tomo_lsqr_create_factored(ctypes.byref(h), int(npairs), int(nper), int(nnodes), int(nz), _ptr(d_lptr), _ptr(d_lnode),
+                                          _ptr(d_lw), int(klen), _ptr(d_kj0), _ptr(d_kern), int(ms), int(snnz), _ptr(d_sptr),
+                                          _ptr(d_sidx), _ptr(d_svals), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_create_factored")
     return h.value
 
 
@@ -285,6 +297,21 @@ class TomoLsqr:
         self._keep = (rowptr.contiguous(), colind.contiguous(), vals.contiguous())
         vt = TOMO_VAL_F64 if vals.dtype == torch.float64 else TOMO_VAL_F32
         self.h = tomo_lsqr_create(self.m, self.n, self.nnz, *self._keep, vt, stream)
+
+    @classmethod
+    def factored(cls, npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None, sidx=None, svals=None, stream=None):
+        """A handle on the factored operator (tomo_lsqr_create_factored); keeps the borrowed device tensors alive."""
+        self = cls.__new__(cls)
+        klen = int(kern.numel()) // int(nper)
+        ms = 0 if sptr is None else int(sptr.numel()) - 1
+        snnz = 0 if sidx is None else int(sidx.numel())
+        keep = [None if t is None else t.contiguous() for t in (lptr, lnode, lw, kj0, kern, sptr, sidx, svals)]
+        self._keep = tuple(keep)
+        self.m, self.n = int(npairs) * int(nper) + ms, int(nnodes) * int(nz)
+        self.nnz = int(lnode.numel()) * int(nper) * klen + snnz
+        self.h = tomo_lsqr_create_factored(npairs, nper, nnodes, nz, keep[0], keep[1], keep[2], klen, keep[3], keep[4], ms, snnz,
+                                           keep[5], keep[6], keep[7], stream)
+        return self
 
     def set(self, **opts):
         for k, v in opts.items():

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtomolsqr.so")
 SOURCES = ["tomo_lsqr.cu"]
-HEADERS = ["accum.cuh", "state.cuh", "tails.cuh", "kernels.cuh", "wstream.cuh", "compress.cuh", "wspmm.cuh", "shard.cuh", "multi.cuh", "build.cuh", os.path.join("..", "..", "include", "tomo_lsqr.h")]
+HEADERS = ["accum.cuh", "state.cuh", "tails.cuh", "kernels.cuh", "wstream.cuh", "compress.cuh", "wspmm.cuh", "shard.cuh", "multi.cuh", "build.cuh", "factored.cuh", os.path.join("..", "..", "include", "tomo_lsqr.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",

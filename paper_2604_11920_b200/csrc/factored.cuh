@@ -1,0 +1,321 @@
+// factored.cuh — the sensitivity block of A in the factored form of PAPER.md Eq. 5 with the depth-fastest
+// unknown ordering of Eq. 7: SURVEY.md §8(f) NEXT-2, second form.
+//
+//   A = [ A_data ; A_extra ],   A_data[(q, p), (k, j)] = fl( W[q, k] * g_p[j - j0_p] )   for j0_p <= j < j0_p + klen,
+//
+// q = station pair (ray), p = period, k = lateral node, j = layer; row q * nper + p, column k * nz + j.  W (npairs x
+// nnodes, the ray's lateral footprint) is a small CSR matrix, g_p the depth kernel of period p on its window of klen
+// layers; A_extra (the smoothing rows) is an ordinary CSR block.  Nothing of A_data is stored per nonzero: a lateral
+// entry (12 bytes) stands for nper * klen nonzeros of the CSR form (12 bytes each), so the operator lives in L2 and the
+// products are bound by arithmetic, not by HBM.  Every product  fl(W g) * x  is formed from the ROUNDED value
+// fl(W g), i.e. from exactly the number the CSR form stores, so in dd mode (order-independent sums, accum.cuh) the
+// results are bit for bit those of the CSR path on the expanded matrix.
+//
+// Lane layout of both kernels: 32 lanes = G groups of nper lanes (G = 32 / nper; the 32 - G * nper last lanes idle).
+// Lane (g, p) keeps the klen kernel values of ITS period in registers and walks the lateral entries g, g + G, ...
+//   k_fac_rows (A x):   one accumulator per lane (row (q, p)); per entry klen gathers of x[k * nz + j0_p + t].
+//   k_fac_cols (A^T x): klen accumulators per lane (layers j0_p .. j0_p + klen - 1 of node k); per entry ONE gather
+//                       x[q * nper + p]; the layer sums of a node are put together through shared memory.
+// Warps own static ranges (pairs balanced by entry count; lateral-CSC entries split evenly, a node cut by a range
+// boundary leaves unrounded (hi, lo) partials and the last warp to arrive closes the node in slot order), so both
+// modes are deterministic.
+#pragma once
+#include "accum.cuh"
+#include "state.cuh"
+#include "tails.cuh"
+
+namespace tomo {
+
+constexpr int kFacWarps = 16;
+constexpr int kFacThreads = kFacWarps * 32;
+
+struct FacSeg {        // one piece of a node's lateral-CSC entry list, owned by one warp
+  int64_t e0, e1;      // entries [e0, e1) of the lateral CSC
+  int32_t node;
+  int32_t nsegs;       // pieces of this node (1: the warp closes the node from its registers)
+  int32_t slot;        // nsegs > 1: where this piece's nz partial pairs go (seg_part + slot * nz); slot0 = slot - rank
+  int32_t rank;        // index of the piece inside its node
+};
+
+struct FacDesc {       // uniform kernel argument
+  int32_t nper, nz, klen, G;
+  int64_t npairs, nnodes, mdata, ms;
+  const int64_t* lptr; const int32_t* lnode; const double* lw;       // W as CSR (pairs x nodes)
+  const int64_t* cptr; const int32_t* cpair; const double* cw;       // W as CSC (pairs ascending inside a node)
+  const int32_t* kj0; const double* kern;                            // [nper], [nper * klen]
+  const int64_t* sptr; const int32_t* sidx; const double* sval;      // A_extra as CSR (ms x n); NULL if ms == 0
+  const int64_t* scptr; const int32_t* srow; const double* scval;    // A_extra as CSC; NULL if it has no entries
+  const int32_t* pw;       // k_fac_rows: first pair of every warp [NW + 1]
+  const int32_t* wseg;     // k_fac_cols: first piece of every warp [NW + 1]
+  const FacSeg* seg;
+  double2* seg_part;       // unrounded partial layer sums of the pieces of cut nodes
+  unsigned int* node_cnt;  // arrivals per cut node; zero between launches
+  double2* node_nsq;       // per node: sum of the squares of its nz results (unrounded pair), summed in node order by the last CTA
+};
+
+template <int MODE>
+__device__ __forceinline__ Acc<MODE> fac_acc_of(double2 p) { Acc<MODE> r; r.unpack(p); return r; }
+
+// y_r <- sum + c * yo  (+ running ||y||^2): the fused axpy + norm of K1 / K2 (as finish_row_with in wstream.cuh)
+template <int MODE, bool AXPY, bool NORM>
+__device__ __forceinline__ double fac_finish(Acc<MODE> sum, double c, double yo, Acc<MODE>& nsq) {
+  double yn;
+  if (AXPY) {
+    if (MODE == 0) yn = fma(c, yo, sum.value());
+    else { sum.mac(c, yo); yn = sum.value(); }
+  } else {
+    yn = sum.value();
+  }
+  if (NORM) nsq.mac(yn, yn);
+  return yn;
+}
+
+// the block's partial of the squared norm -> partials[blockIdx.x]; the last CTA returns true
+__device__ __forceinline__ bool fac_ticket(Scalars* sc, int* s_flag) {
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned int t = atomicAdd(&sc->ticket[0], 1u);
+    *s_flag = (t == gridDim.x - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  const bool last = *s_flag != 0;
+  if (last) __threadfence();
+  return last;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// A x over the pairs:  OP_PLAIN  y = A x ;  OP_K1  u^ = A v - alpha u (u = u^ * rbeta applied where read), ||u^||^2, tail
+// ------------------------------------------------------------------------------------------------------------------
+template <int MODE, int OP, int KLP, bool GUARD>
+__global__ void __launch_bounds__(GUARD ? kFacThreads / 2 : kFacThreads, 1)
+k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
+  __shared__ double2 s_slots[kFacWarps];
+  __shared__ int s_flag;
+  constexpr bool K1 = (OP == OP_K1);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nwarp = blockDim.x >> 5;   // 16, or 8 in the general-window shape (twice the CTAs, same warp numbering)
+  const int gw = blockIdx.x * nwarp + warp, NW = gridDim.x * nwarp;
+  const int nper = d.nper, G = d.G, klen = GUARD ? d.klen : KLP;
+  const int p = lane % nper, g = lane / nper;
+  const bool active = g < G;
+
+  // ---- prologue: nothing the previous kernel writes ----
+  double kr[KLP];
+#pragma unroll
+  for (int t = 0; t < KLP; ++t) kr[t] = (!GUARD || t < klen) ? d.kern[(size_t)p * klen + t] : 0.0;
+  const int j0 = d.kj0[p];
+  const int q0 = d.pw[gw], q1 = d.pw[gw + 1];
+  const int64_t x0 = d.ms * gw / NW, x1 = d.ms * (int64_t)(gw + 1) / NW;  // this warp's share of the extra rows
+
+  grid_dependency_wait();
+  double c = 0.0, sy = 1.0;
+  if (K1) {
+    if (sc->stop) return;
+    c = -sc->alpha; sy = sc->rbeta;
+  }
+  Acc<MODE> nsq;
+  nsq.zero();
+
+  for (int q = q0; q < q1; ++q) {
+    const int64_t e0 = d.lptr[q], e1 = d.lptr[q + 1];
+    Acc<MODE> a0, a1;
+    a0.zero(); a1.zero();
+    if (active) {
+      int64_t e = e0 + g;
+      bool has = e < e1;
+      int k = has ? d.lnode[e] : 0;
+      double w = has ? d.lw[e] : 0.0;
+      while (has) {
+        const double* xp = x + (int64_t)k * d.nz + j0;
+        double xv[KLP];
+#pragma unroll
+        for (int t = 0; t < KLP; ++t) xv[t] = (!GUARD || t < klen) ? xp[t] : 0.0;
+        const double wc = w;
+        e += G;
+        has = e < e1;
+        if (has) { k = d.lnode[e]; w = d.lw[e]; }   // the next entry is on its way while this one is summed
+#pragma unroll
+        for (int t = 0; t < KLP; t += 2) {
+          if (!GUARD || t < klen) a0.mac(wc * kr[t], xv[t]);
+          if (t + 1 < KLP && (!GUARD || t + 1 < klen)) a1.mac(wc * kr[t + 1], xv[t + 1]);
+        }
+      }
+    }
+    a0.merge(a1);
+    for (int gg = 1; gg < G; ++gg) {      // groups in index order (fixed): lane p collects lanes p + gg * nper
+      const Acc<MODE> o = a0.down(gg * nper);
+      if (g == 0) a0.merge(o);
+    }
+    if (lane < nper) {
+      const int64_t r = (int64_t)q * nper + lane;
+      const double yo = K1 ? y[r] * sy : 0.0;
+      y[r] = fac_finish<MODE, K1, K1>(a0, c, yo, nsq);
+    }
+  }
+  // the extra (smoothing) rows: one lane per row, entries in order
+  for (int64_t r = x0 + lane; r < x1; r += 32) {
+    Acc<MODE> a;
+    a.zero();
+    for (int64_t e = d.sptr[r]; e < d.sptr[r + 1]; ++e) a.mac(d.sval[e], x[d.sidx[e]]);
+    const int64_t ro = d.mdata + r;
+    const double yo = K1 ? y[ro] * sy : 0.0;
+    y[ro] = fac_finish<MODE, K1, K1>(a, c, yo, nsq);
+  }
+  if (!K1) return;
+
+  lanes_reduce<32, MODE>(nsq);
+  if (lane == 0) s_slots[warp] = nsq.pack();
+  __syncthreads();
+  grid_launch_dependents();
+  if (threadIdx.x == 0) {
+    Acc<MODE> tot = fac_acc_of<MODE>(s_slots[0]);
+    for (int i = 1; i < nwarp; ++i) tot.merge(fac_acc_of<MODE>(s_slots[i]));
+    __stcg(partials + blockIdx.x, tot.pack());
+  }
+  if (!fac_ticket(sc, &s_flag)) return;
+  const double total = final_sum<MODE>(partials, (int)gridDim.x, s_slots);
+  if (threadIdx.x == 0) {
+    tail_k1(sc, total);
+    sc->ticket[0] = 0u;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// A^T x over the lateral CSC:  OP_PLAIN  y = A^T x ;  OP_K2  v^ = A^T u - beta v, ||v^||^2, tail ;  OP_K2_INIT (no axpy)
+// ------------------------------------------------------------------------------------------------------------------
+template <int MODE, int OP, int KLP, bool GUARD>
+__global__ void __launch_bounds__(GUARD ? kFacThreads / 2 : kFacThreads, 1)
+k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
+  extern __shared__ __align__(16) unsigned char fac_smem[];
+  __shared__ double2 s_slots[kFacWarps];
+  __shared__ int s_kj0[32];
+  __shared__ int s_flag;
+  constexpr bool NORM = (OP != OP_PLAIN), AXPY = (OP == OP_K2), SCALE = (OP != OP_PLAIN);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int gw = blockIdx.x * (blockDim.x >> 5) + warp;
+  const int nper = d.nper, G = d.G, nz = d.nz, klen = GUARD ? d.klen : KLP;
+  const int p = lane % nper, g = lane / nper;
+  const bool active = g < G;
+  double2* my = reinterpret_cast<double2*>(fac_smem) + (size_t)warp * 32 * KLP;   // [t][lane]
+
+  double kr[KLP];
+#pragma unroll
+  for (int t = 0; t < KLP; ++t) kr[t] = (!GUARD || t < klen) ? d.kern[(size_t)p * klen + t] : 0.0;
+  if (threadIdx.x < 32) s_kj0[threadIdx.x] = (threadIdx.x < nper) ? d.kj0[threadIdx.x] : 0;
+  const int s0 = d.wseg[gw], s1 = d.wseg[gw + 1];
+  __syncthreads();
+
+  grid_dependency_wait();
+  double c = 0.0, sx = 1.0;
+  if (OP != OP_PLAIN) {
+    if (sc->stop) return;
+    if (OP == OP_K2 && sc->beta_zero) {   // beta = 0: the A^T pass is skipped, the scalar step still runs
+      if (blockIdx.x == 0 && threadIdx.x == 0) tail_k2(sc, 0.0);
+      return;
+    }
+    if (OP == OP_K2) c = -sc->beta;
+    sx = sc->rbeta;
+  }
+
+  for (int s = s0; s < s1; ++s) {
+    const FacSeg sg = d.seg[s];
+    Acc<MODE> acc[KLP];
+#pragma unroll
+    for (int t = 0; t < KLP; ++t) acc[t].zero();
+    if (active) {
+      int64_t e = sg.e0 + g;
+      bool has = e < sg.e1;
+      int q = has ? d.cpair[e] : 0;
+      double w = has ? d.cw[e] : 0.0;
+      double xs = has ? x[(int64_t)q * nper + p] : 0.0;
+      while (has) {
+        const double wc = w;
+        const double us = SCALE ? xs * sx : xs;
+        e += G;
+        has = e < sg.e1;
+        if (has) { q = d.cpair[e]; w = d.cw[e]; xs = x[(int64_t)q * nper + p]; }
+#pragma unroll
+        for (int t = 0; t < KLP; ++t)
+          if (!GUARD || t < klen) acc[t].mac(wc * kr[t], us);
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < KLP; ++t) my[t * 32 + lane] = acc[t].pack();
+    __syncwarp();
+    const int node = sg.node;
+    const bool whole = sg.nsegs == 1;
+    Acc<MODE> nsq;
+    nsq.zero();
+    // the closing of layer j of this node: the extra rows' column, the axpy, the rounding, the norm
+    auto close = [&](int j, Acc<MODE> S) {
+      const int64_t col = (int64_t)node * nz + j;
+      if (d.scptr) {
+        for (int64_t e = d.scptr[col]; e < d.scptr[col + 1]; ++e) {
+          const double xe = x[d.mdata + d.srow[e]];
+          S.mac(d.scval[e], SCALE ? xe * sx : xe);
+        }
+      }
+      const double yo = AXPY ? y[col] : 0.0;
+      y[col] = fac_finish<MODE, AXPY, NORM>(S, c, yo, nsq);
+    };
+    for (int j = lane; j < nz; j += 32) {   // layer sums over periods (ascending) and groups (ascending): fixed order
+      Acc<MODE> S;
+      S.zero();
+      for (int pp = 0; pp < nper; ++pp) {
+        const int t = j - s_kj0[pp];
+        if (t >= 0 && t < klen)
+          for (int gg = 0; gg < G; ++gg) S.merge(fac_acc_of<MODE>(my[t * 32 + gg * nper + pp]));
+      }
+      if (whole) close(j, S);
+      else __stcg(d.seg_part + (size_t)sg.slot * nz + j, S.pack());
+    }
+    bool closer = whole;
+    if (!whole) {
+      __threadfence();
+      __syncwarp();
+      unsigned int old = 0;
+      if (lane == 0) old = atomicAdd(d.node_cnt + node, 1u);
+      old = __shfl_sync(0xffffffffu, old, 0);
+      if (old == (unsigned int)(sg.nsegs - 1)) {    // every other piece of the node has been published
+        __threadfence();
+        closer = true;
+        if (lane == 0) d.node_cnt[node] = 0u;
+        const double2* base = d.seg_part + (size_t)(sg.slot - sg.rank) * nz;
+        for (int j = lane; j < nz; j += 32) {
+          Acc<MODE> S = fac_acc_of<MODE>(__ldcg(base + j));
+          for (int r = 1; r < sg.nsegs; ++r) S.merge(fac_acc_of<MODE>(__ldcg(base + (size_t)r * nz + j)));
+          close(j, S);
+        }
+      }
+    }
+    if (NORM && closer) {
+      lanes_reduce<32, MODE>(nsq);
+      if (lane == 0) { __stcg(d.node_nsq + node, nsq.pack()); __threadfence(); }
+    }
+    __syncwarp();
+  }
+  if (!NORM) return;
+
+  __syncthreads();
+  grid_launch_dependents();
+  if (!fac_ticket(sc, &s_flag)) return;
+  const double total = final_sum<MODE>(d.node_nsq, (int)d.nnodes, s_slots);
+  if (threadIdx.x == 0) {
+    if (OP == OP_K2) tail_k2(sc, total);
+    if (OP == OP_K2_INIT) tail_init_v(sc, total);
+    sc->ticket[0] = 0u;
+  }
+}
+
+// validation of the depth-kernel table: windows inside [0, nz), finite values
+__global__ void k_fac_validate_kern(int nper, int nz, int klen, const int32_t* __restrict__ kj0, const double* __restrict__ kern,
+                                    int* flags) {
+  int bad = 0;
+  for (int i = threadIdx.x; i < nper; i += blockDim.x)
+    if (kj0[i] < 0 || kj0[i] + klen > nz) bad = 1;
+  for (int i = threadIdx.x; i < nper * klen; i += blockDim.x)
+    if (!(fabs(kern[i]) <= 1.79769313486231570815e308)) bad = 1;
+  if (bad) atomicOr(flags, 1);
+}
+
+}  // namespace tomo

@@ -21,6 +21,7 @@
 #include "compress.cuh"
 #include "shard.cuh"
 #include "multi.cuh"
+#include "factored.cuh"
 
 using namespace tomo;
 
@@ -67,8 +68,22 @@ struct Dir {
   unsigned char* cidx = nullptr; int64_t* coff = nullptr; int64_t cbytes = 0, heads = 0;  // run-compressed index (FMT 1)
 };
 
+// the factored sensitivity block (factored.cuh; tomo_lsqr_create_factored): what the handle owns of it
+struct FacState {
+  FacDesc d = {};                 // the kernel argument (borrowed W / A_extra CSR arrays, owned rest)
+  int64_t E = 0, snnz = 0;        // lateral entries, entries of the extra rows
+  int klp = 0; bool guard = false;  // kernel shape: window length as a template constant (8, 12, 16) or the general one (32, guarded)
+  int nsegs = 0, nslots = 0;
+  int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
+  int32_t* kj0 = nullptr; double* kern = nullptr;
+  int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
+  int32_t* pw = nullptr; int32_t* wseg = nullptr; FacSeg* seg = nullptr;
+  double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr;
+};
+
 struct tomo_lsqr_s {
   int64_t m = 0, n = 0, nnz = 0;
+  FacState* fac = nullptr;               // non-NULL: A is held in factored form, the CSR / CSC members below are unused
   int device = 0;                        // the device the handle was created on; every call checks it is current
   tomo_valtype_t vt = TOMO_VAL_F64;
   // borrowed CSR
@@ -195,8 +210,68 @@ void launch_wstream_dir(const tomo_lsqr_s* h, bool transpose, const double* x, d
   else launch_wstream_t<MODE, VT, OP_PLAIN, FMT, false>(h, x, y, st);
 }
 
+// ---- factored operator (factored.cuh): launch shapes ----
+template <int KLP, bool GUARD> constexpr size_t fac_cols_smem() { return (size_t)(GUARD ? kFacWarps / 2 : kFacWarps) * 32 * KLP * sizeof(double2); }
+
+template <int MODE, int OP, int KLP, bool GUARD>
+cudaError_t launch_fac_one(const tomo_lsqr_s* h, bool cols, const double* x, double* y, cudaStream_t st) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(GUARD ? 2 * h->sms : h->sms));
+  cfg.blockDim = dim3(GUARD ? kFacThreads / 2 : kFacThreads);
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = (h->pdl && OP != OP_PLAIN) ? 1 : 0;
+  if (cols) {
+    if constexpr (OP == OP_PLAIN || OP == OP_K2 || OP == OP_K2_INIT) {
+      cfg.dynamicSmemBytes = fac_cols_smem<KLP, GUARD>();
+      return cudaLaunchKernelEx(&cfg, k_fac_cols<MODE, OP, KLP, GUARD>, h->fac->d, x, y, h->sc, h->part_spmv);
+    }
+  } else {
+    if constexpr (OP == OP_PLAIN || OP == OP_K1) {
+      cfg.dynamicSmemBytes = 0;
+      return cudaLaunchKernelEx(&cfg, k_fac_rows<MODE, OP, KLP, GUARD>, h->fac->d, x, y, h->sc, h->part_spmv);
+    }
+  }
+  return cudaErrorInvalidValue;
+}
+template <int MODE, int OP>
+cudaError_t launch_fac_mode(const tomo_lsqr_s* h, bool cols, const double* x, double* y, cudaStream_t st) {
+  switch (h->fac->klp) {
+    case 8: return launch_fac_one<MODE, OP, 8, false>(h, cols, x, y, st);
+    case 12: return launch_fac_one<MODE, OP, 12, false>(h, cols, x, y, st);
+    case 16: return launch_fac_one<MODE, OP, 16, false>(h, cols, x, y, st);
+    default: return launch_fac_one<MODE, OP, 32, true>(h, cols, x, y, st);
+  }
+}
+template <int OP>
+void launch_fac(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  if (h->accumulate) launch_fac_mode<1, OP>(h, transpose, x, y, st);
+  else launch_fac_mode<0, OP>(h, transpose, x, y, st);
+}
+// the > 48 KB dynamic shared memory opt-in of the k_fac_cols instantiations on the current device
+template <int MODE, int KLP, bool GUARD>
+cudaError_t fac_attr_one() {
+  cudaError_t e;
+  const int b = (int)fac_cols_smem<KLP, GUARD>();
+  if ((e = cudaFuncSetAttribute(k_fac_cols<MODE, OP_PLAIN, KLP, GUARD>, cudaFuncAttributeMaxDynamicSharedMemorySize, b)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_fac_cols<MODE, OP_K2, KLP, GUARD>, cudaFuncAttributeMaxDynamicSharedMemorySize, b)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_fac_cols<MODE, OP_K2_INIT, KLP, GUARD>, cudaFuncAttributeMaxDynamicSharedMemorySize, b);
+}
+cudaError_t set_fac_attributes(int klp) {
+  cudaError_t e;
+  switch (klp) {
+    case 8: if ((e = fac_attr_one<0, 8, false>()) != cudaSuccess) return e; return fac_attr_one<1, 8, false>();
+    case 12: if ((e = fac_attr_one<0, 12, false>()) != cudaSuccess) return e; return fac_attr_one<1, 12, false>();
+    case 16: if ((e = fac_attr_one<0, 16, false>()) != cudaSuccess) return e; return fac_attr_one<1, 16, false>();
+    default: if ((e = fac_attr_one<0, 32, true>()) != cudaSuccess) return e; return fac_attr_one<1, 32, true>();
+  }
+}
+
 template <int OP>
 void launch_spmv(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  if (h->fac) { launch_fac<OP>(h, transpose, x, y, st); return; }
   const bool cz = h->compress && h->dir[transpose ? 1 : 0].cidx;
   if (h->vt == TOMO_VAL_F64) {
     if (h->accumulate) { if (cz) launch_wstream_dir<1, double, OP, 1>(h, transpose, x, y, st); else launch_wstream_dir<1, double, OP, 0>(h, transpose, x, y, st); }
@@ -393,6 +468,12 @@ void free_handle(tomo_lsqr_s* h) {
   cudaFree(h->mU); cudaFree(h->mV); cudaFree(h->mW); cudaFree(h->mX); cudaFree(h->mH); cudaFree(h->msc); cudaFree(h->cta_rec8);
   cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->h_mpoll) cudaFreeHost(h->h_mpoll); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
+  if (FacState* f = h->fac) {
+    cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->wseg); cudaFree(f->seg);
+    cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq);
+    delete f;
+  }
   cudaFree(h->cta_rec);
   cudaFree(h->u); cudaFree(h->v); cudaFree(h->w); cudaFree(h->x); cudaFree(h->hbar);
   cudaFree(h->sc); cudaFree(h->part_spmv); cudaFree(h->part_vec);
@@ -485,6 +566,190 @@ extern "C" tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   if (e2) cudaEventDestroy(e2);
+  if (rc != TOMO_OK) { free_handle(h); return rc; }
+  *out = h;
+  return TOMO_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-2, factored form (factored.cuh): create
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+// CSR -> CSC of a small block with the transpose passes of build.cuh (a temporary handle carries the arguments)
+tomo_status_t transpose_block(int sms, int64_t m, int64_t n, int64_t nnz, const int64_t* ptr, const int32_t* idx, const double* val,
+                              cudaStream_t st, int64_t** cptr, int32_t** cidx, double** cval) {
+  tomo_lsqr_s t;
+  t.m = m; t.n = n; t.nnz = nnz; t.sms = sms; t.rowptr = ptr; t.colind = idx; t.vals = val;
+  tomo_status_t rc = build_csc<double>(&t, st, false);
+  if (rc != TOMO_OK) { cudaFree(t.colptr); cudaFree(t.rowind); cudaFree(t.cvals); return rc; }
+  *cptr = t.colptr; *cidx = t.rowind; *cval = (double*)t.cvals;
+  return TOMO_OK;
+}
+
+}  // namespace
+
+extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz,
+                                                   const int64_t* d_lptr, const int32_t* d_lnode, const double* d_lw,
+                                                   int32_t klen, const int32_t* d_kj0, const double* d_kern, int64_t ms,
+                                                   int64_t snnz, const int64_t* d_sptr, const int32_t* d_sidx,
+                                                   const double* d_svals, void* cuda_stream) {
+  if (!out) return TOMO_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (npairs < 1 || nnodes < 1 || nz < 1 || nper < 1 || klen < 1 || ms < 0 || snnz < 0) return TOMO_ERR_INVALID_ARG;
+  if (nper > 32 || klen > 32 || klen > nz) return TOMO_ERR_RANGE;
+  if ((double)npairs * nper + (double)ms >= (double)INT32_MAX || (double)nnodes * nz >= (double)INT32_MAX) return TOMO_ERR_RANGE;
+  if (!d_lptr || !d_kj0 || !d_kern || (ms > 0 && !d_sptr) || (snnz > 0 && (!d_sidx || !d_svals || ms == 0))) return TOMO_ERR_INVALID_ARG;
+  int dev = 0, major = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) return TOMO_ERR_UNSUPPORTED_ARCH;
+  if (!is_device_ptr(d_lptr) || !is_device_ptr(d_kj0) || !is_device_ptr(d_kern) || (ms > 0 && !is_device_ptr(d_sptr)) ||
+      (snnz > 0 && (!is_device_ptr(d_sidx) || !is_device_ptr(d_svals))))
+    return TOMO_ERR_NOT_DEVICE_PTR;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t m = npairs * nper + ms, n = nnodes * nz;
+
+  // the pair pointer array on the host: the number of lateral entries and the warps' pair ranges come from it
+  std::vector<int64_t> lptr((size_t)npairs + 1);
+  CK(cudaMemcpyAsync(lptr.data(), d_lptr, sizeof(int64_t) * (npairs + 1), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const int64_t E = lptr[npairs];
+  if (lptr[0] != 0 || E < 0 || E >= ((int64_t)1 << 40)) return TOMO_ERR_BAD_CSR;
+  for (int64_t q = 0; q < npairs; ++q) if (lptr[q] > lptr[q + 1]) return TOMO_ERR_BAD_CSR;
+  if (E > 0 && (!d_lnode || !d_lw)) return TOMO_ERR_INVALID_ARG;
+  if (E > 0 && (!is_device_ptr(d_lnode) || !is_device_ptr(d_lw))) return TOMO_ERR_NOT_DEVICE_PTR;
+
+  tomo_lsqr_s* h = new (std::nothrow) tomo_lsqr_s();
+  FacState* f = new (std::nothrow) FacState();
+  if (!h || !f) { delete h; delete f; return TOMO_ERR_OOM; }
+  h->fac = f;
+  h->m = m; h->n = n; h->nnz = E * nper * klen + snnz; h->vt = TOMO_VAL_F64; h->sms = sms; h->device = dev;
+  h->SG = sms; h->part_dirty = false;
+  f->E = E; f->snnz = snnz;
+  f->klp = (klen == 8 || klen == 12 || klen == 16) ? klen : 32;
+  f->guard = f->klp == 32;
+  const int NW = sms * kFacWarps;
+
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  tomo_status_t rc = TOMO_OK;
+  int* d_flags = nullptr;
+  do {
+    cudaError_t e;
+    if ((e = set_fac_attributes(f->klp)) != cudaSuccess) { rc = cuda_fail(e, "cudaFuncSetAttribute(shared memory opt-in)"); break; }
+    if ((e = cudaEventCreate(&e0)) != cudaSuccess || (e = cudaEventCreate(&e1)) != cudaSuccess) { rc = cuda_fail(e, "cudaEventCreate"); break; }
+    cudaEventRecord(e0, st);
+    // --- validation: W and A_extra as canonical CSR blocks, the kernel table ---
+    if ((e = cudaMalloc(&d_flags, sizeof(int))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc"); break; }
+    cudaMemsetAsync(d_flags, 0, sizeof(int), st);
+    k_validate<double><<<sms * 8, kThreads, 0, st>>>(npairs, nnodes, E, d_lptr, d_lnode, d_lw, d_flags);
+    if (ms > 0) k_validate<double><<<sms * 8, kThreads, 0, st>>>(ms, n, snnz, d_sptr, d_sidx, d_svals, d_flags);
+    k_fac_validate_kern<<<1, 256, 0, st>>>(nper, nz, klen, d_kj0, d_kern, d_flags);
+    int flags = 0;
+    if ((e = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "validation of the factored operator"); break; }
+    if (flags) { rc = TOMO_ERR_BAD_CSR; break; }
+    // --- the transposes: W by node, A_extra by column ---
+    if ((rc = transpose_block(sms, npairs, nnodes, E, d_lptr, d_lnode, d_lw, st, &f->cptr, &f->cpair, &f->cw)) != TOMO_OK) break;
+    if (snnz > 0 && (rc = transpose_block(sms, ms, n, snnz, d_sptr, d_sidx, d_svals, st, &f->scptr, &f->srow, &f->scval)) != TOMO_OK) break;
+#define ALLOC(p, bytes) if ((e = cudaMalloc(&(p), (bytes))) != cudaSuccess) { rc = cuda_fail(e, "cudaMalloc(factored)"); break; }
+    ALLOC(f->kj0, sizeof(int32_t) * nper); ALLOC(f->kern, sizeof(double) * nper * klen);
+    if ((e = cudaMemcpyAsync(f->kj0, d_kj0, sizeof(int32_t) * nper, cudaMemcpyDeviceToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(f->kern, d_kern, sizeof(double) * nper * klen, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the kernel table"); break; }
+    // --- static work split (host): pairs by entry count for A x; lateral-CSC entries cut evenly for A^T x ---
+    const int G = 32 / nper;
+    std::vector<int32_t> pw((size_t)NW + 1);
+    {
+      // cost of a pair in lane steps: ceil(entries / G) + 4 (group combine, row stores)
+      std::vector<double> pre((size_t)npairs + 1, 0.0);
+      for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 4.0;
+      int64_t q = 0;
+      pw[0] = 0;
+      for (int w = 1; w < NW; ++w) {
+        const double target = pre[npairs] * (double)w / (double)NW;
+        while (q < npairs && 0.5 * (pre[q] + pre[q + 1]) < target) ++q;
+        pw[w] = (int32_t)q;
+      }
+      pw[NW] = (int32_t)npairs;
+    }
+    std::vector<int64_t> cptr((size_t)nnodes + 1);
+    if ((e = cudaMemcpyAsync(cptr.data(), f->cptr, sizeof(int64_t) * (nnodes + 1), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the node pointers"); break; }
+    std::vector<FacSeg> segs;
+    std::vector<int32_t> wseg((size_t)NW + 1, 0), owner;
+    {
+      auto bound = [&](int w) { return (int64_t)((double)E * (double)w / (double)NW); };   // first entry of warp w's range
+      int w = 0, nslots = 0;
+      for (int64_t k = 0; k < nnodes; ++k) {
+        const int64_t lo = cptr[k], hi = cptr[k + 1];
+        const size_t first = segs.size();
+        if (lo == hi) {
+          if (E == 0) w = (int)(k * NW / nnodes);
+          else while (w + 1 < NW && bound(w + 1) <= lo) ++w;
+          segs.push_back(FacSeg{lo, lo, (int32_t)k, 1, 0, 0}); owner.push_back(w);
+        } else {
+          int64_t a = lo;
+          while (a < hi) {
+            while (w + 1 < NW && bound(w + 1) <= a) ++w;
+            const int64_t b = (w + 1 < NW) ? std::min(hi, std::max(bound(w + 1), a + 1)) : hi;
+            segs.push_back(FacSeg{a, b, (int32_t)k, 1, 0, 0}); owner.push_back(w);
+            a = b;
+          }
+        }
+        const int cnt = (int)(segs.size() - first);
+        if (cnt > 1) {
+          for (int r = 0; r < cnt; ++r) { segs[first + r].nsegs = cnt; segs[first + r].rank = r; segs[first + r].slot = nslots + r; }
+          nslots += cnt;
+        }
+      }
+      for (size_t i = 0; i < segs.size(); ++i) wseg[(size_t)owner[i] + 1] += 1;
+      for (int i = 0; i < NW; ++i) wseg[i + 1] += wseg[i];
+      f->nsegs = (int)segs.size(); f->nslots = nslots;
+    }
+    ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->wseg, sizeof(int32_t) * (NW + 1));
+    ALLOC(f->seg, sizeof(FacSeg) * std::max<size_t>(segs.size(), 1));
+    ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(f->nslots, 1) * nz);
+    ALLOC(f->node_cnt, sizeof(unsigned int) * nnodes); ALLOC(f->node_nsq, sizeof(double2) * nnodes);
+    if ((e = cudaMemcpyAsync(f->pw, pw.data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(f->wseg, wseg.data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(f->seg, segs.data(), sizeof(FacSeg) * segs.size(), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemsetAsync(f->node_cnt, 0, sizeof(unsigned int) * nnodes, st)) != cudaSuccess ||
+        (e = cudaMemsetAsync(f->node_nsq, 0, sizeof(double2) * nnodes, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the work split"); break; }
+    // --- work space (as tomo_lsqr_create) ---
+    h->part_cap = sms * 32 + 2;
+    ALLOC(h->u, sizeof(double) * m); ALLOC(h->v, sizeof(double) * n);
+    ALLOC(h->w, sizeof(double) * n); ALLOC(h->x, sizeof(double) * n);
+    ALLOC(h->sc, sizeof(Scalars));
+    ALLOC(h->part_spmv, sizeof(double2) * h->part_cap);
+    ALLOC(h->part_vec, sizeof(double2) * h->part_cap);
+#undef ALLOC
+    if ((e = cudaMemsetAsync(h->sc, 0, sizeof(Scalars), st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
+    if ((e = cudaMallocHost(&h->h_sc, sizeof(Scalars))) != cudaSuccess ||
+        (e = cudaMallocHost(&h->h_poll, 2 * sizeof(PollWord))) != cudaSuccess) { rc = cuda_fail(e, "cudaMallocHost"); break; }
+    for (int i = 0; i < 2; ++i)
+      if ((e = cudaEventCreateWithFlags(&h->ev_poll[i], cudaEventDisableTiming)) != cudaSuccess) break;
+    if (e != cudaSuccess) { rc = cuda_fail(e, "cudaEventCreate"); break; }
+    if ((e = cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = cuda_fail(e, "cudaStreamCreate"); break; }
+    FacDesc& d = f->d;
+    d.nper = nper; d.nz = nz; d.klen = klen; d.G = G;
+    d.npairs = npairs; d.nnodes = nnodes; d.mdata = npairs * nper; d.ms = ms;
+    d.lptr = d_lptr; d.lnode = d_lnode; d.lw = d_lw;
+    d.cptr = f->cptr; d.cpair = f->cpair; d.cw = f->cw;
+    d.kj0 = f->kj0; d.kern = f->kern;
+    d.sptr = d_sptr; d.sidx = d_sidx; d.sval = d_svals;
+    d.scptr = f->scptr; d.srow = f->srow; d.scval = f->scval;
+    d.pw = f->pw; d.wseg = f->wseg; d.seg = f->seg;
+    d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq;
+    cudaEventRecord(e1, st);
+    if ((e = cudaEventSynchronize(e1)) != cudaSuccess) { rc = cuda_fail(e, "create_factored"); break; }
+    float msf = 0;
+    cudaEventElapsedTime(&msf, e0, e1); h->create_ms = msf;
+  } while (0);
+  if (d_flags) cudaFree(d_flags);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
   if (rc != TOMO_OK) { free_handle(h); return rc; }
   *out = h;
   return TOMO_OK;
@@ -917,7 +1182,7 @@ tomo_status_t solve_multi_any(tomo_lsqr_s* h, int solver, int32_t nrhs, const do
   if (rc != TOMO_OK) return rc;
   if (nrhs < 1 || nrhs > 8 || !d_B || !d_X) return TOMO_ERR_INVALID_ARG;
   if (!is_device_ptr(d_B) || !is_device_ptr(d_X)) return TOMO_ERR_NOT_DEVICE_PTR;
-  if (h->multi_shared) {
+  if (h->multi_shared && !h->fac) {   // a factored handle runs the sides one after the other (no block kernel for it)
     rc = solve_multi_shared(h, solver, nrhs, d_B, damp, atol, btol, max_iters, d_X, res, st);
     h->solver = 0;
     return rc;
@@ -990,7 +1255,7 @@ tomo_status_t update_values_t(tomo_lsqr_s* h, const VT* d_vals, cudaStream_t st)
 }  // namespace
 
 extern "C" tomo_status_t tomo_lsqr_update_values(tomo_lsqr_t h, const void* d_vals, void* cuda_stream) {
-  if (!h || (h->nnz > 0 && !d_vals)) return TOMO_ERR_INVALID_ARG;
+  if (!h || h->fac || (h->nnz > 0 && !d_vals)) return TOMO_ERR_INVALID_ARG;  // a factored handle stores no value per nonzero
   { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
   if (h->nnz > 0 && !is_device_ptr(d_vals)) return TOMO_ERR_NOT_DEVICE_PTR;
   if ((uintptr_t)d_vals & 15u) return TOMO_ERR_INVALID_ARG;
@@ -1100,7 +1365,7 @@ extern "C" tomo_status_t tomo_lsqr_solve_sharded(const tomo_lsqr_t* shards, int3
   if (!is_device_ptr(d_x)) return TOMO_ERR_NOT_DEVICE_PTR;
   for (int l = 0; l < nlocal; ++l) {
     const tomo_lsqr_s* h = shards[l];
-    if (!h || h->n != h0->n || h->vt != h0->vt || h->device != h0->device) return TOMO_ERR_INVALID_ARG;
+    if (!h || h->fac || h->n != h0->n || h->vt != h0->vt || h->device != h0->device) return TOMO_ERR_INVALID_ARG;
     if (!d_b[l]) return TOMO_ERR_INVALID_ARG;
     if (!is_device_ptr(d_b[l])) return TOMO_ERR_NOT_DEVICE_PTR;
   }
@@ -1127,7 +1392,7 @@ extern "C" tomo_status_t tomo_lsqr_spmv(tomo_lsqr_t h, int transpose, const doub
 }
 
 extern "C" tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_rowind, void* d_cvals, void* cuda_stream) {
-  if (!h) return TOMO_ERR_INVALID_ARG;
+  if (!h || h->fac) return TOMO_ERR_INVALID_ARG;
   { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t vb = h->vt == TOMO_VAL_F64 ? sizeof(double) : sizeof(float);
@@ -1148,6 +1413,7 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "multi_shared") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->multi_shared = (int)value; }
   else if (k == "compress") {
     if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG;
+    if (h->fac) return value == 0 ? TOMO_OK : TOMO_ERR_INVALID_ARG;
     { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
     if (value == 1) for (int d = 0; d < 2; ++d) { tomo_status_t rc = build_compressed(h, d, nullptr); if (rc != TOMO_OK) return rc; }
     if (h->compress != (int)value && h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
@@ -1164,6 +1430,13 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   const std::string k(key);
   const double vb = h->vt == TOMO_VAL_F64 ? 8.0 : 4.0;
   if (k == "create_ms") *out = h->create_ms;
+  else if (k == "factored") *out = h->fac ? 1.0 : 0.0;
+  else if (k == "lateral_entries") *out = h->fac ? (double)h->fac->E : 0.0;
+  else if (k == "cut_nodes_pieces") *out = h->fac ? (double)h->fac->nslots : 0.0;
+  else if (k == "operator_bytes")   // what a product has to read of the operator itself
+    *out = h->fac ? 12.0 * (double)h->fac->E + 8.0 * (double)(h->fac->d.npairs + 1) + 12.0 * (double)h->fac->snnz + 8.0 * (double)(h->fac->d.ms + 1)
+                  : (double)h->nnz * (4.0 + vb) + 8.0 * (double)(h->m + 1);
+  else if (h->fac && (k == "csc_bytes" || k.rfind("compress_bytes", 0) == 0 || k.rfind("cta_busy", 0) == 0)) return TOMO_ERR_INVALID_ARG;
   else if (k == "transpose_ms") *out = h->transpose_ms;
   else if (k == "transpose_kernels_ms") *out = h->transpose_kernels_ms;
   else if (k == "update_ms") *out = h->update_ms;

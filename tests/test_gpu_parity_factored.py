@@ -1,0 +1,251 @@
+"""GPU parity of the factored operator (tomo_lsqr_create_factored, second form; Eq. 5
+P:69-71, Eq. 7) through the C ABI against the CPU oracle on the multiplied-out matrix (oracle/factored.py, whose
+output is pinned bitwise to the generator's CSR assembly in tests/test_oracle_factored_pins.py).
+
+Bars: as for the CSR path (north_star): SpMV <= 1e-12, x_50 <= 1e-8; in dd mode the sums are order-independent, so the
+factored kernels (another order of the same rounded products) must reproduce the oracle bit for bit, which is asserted.
+Runs after test_gpu_parity.py (file name), when the full-size oracle jobs have finished.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import oracle_jobs
+import tomogen
+from oracle import factored as ofac
+
+pytestmark = pytest.mark.gpu
+
+TOL_SPMV = 1e-12
+TOL_X50 = 1e-8
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.fixture(scope="module")
+def tl():
+    from paper_2604_11920_b200 import build
+    build.build()
+    import paper_2604_11920_b200 as tl
+    tl.load()
+    return tl
+
+
+def make(tl, f):
+    return tl.TomoLsqr.factored(f["npairs"], f["nper"], f["nnodes"], f["nz"], dev(f["lptr"]), dev(f["lnode"]), dev(f["lw"]),
+                                dev(f["kj0"].astype(np.int32)), dev(f["kern"]), dev(f["sptr"]), dev(f["sidx"]), dev(f["svals"]))
+
+
+def expand(f):
+    return ofac.expand(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                       f["sptr"], f["sidx"], f["svals"])
+
+
+SHAPES = [  # npairs, nper, nnodes, nz, klen, ms   (klen 8 / 12 / 16: the template shapes; others: the general shape)
+    (300, 5, 64, 8, 8, None),      # config-0-like
+    (500, 10, 100, 20, 12, None),  # config-1-like: three groups of ten lanes, two idle
+    (200, 16, 50, 40, 12, None),   # config-2-like: nz > 32 (two layers per lane in the closing)
+    (120, 7, 30, 24, 16, 0),       # no extra block
+    (90, 1, 40, 5, 5, None),       # one period: 32 groups of one lane; window = all layers; general shape
+    (60, 32, 9, 33, 1, 50),        # 32 periods: one group; one-layer windows
+    (150, 3, 2500, 12, 7, None),   # many nodes, most of them with no ray (closed from the extra block alone)
+    (40, 11, 6, 32, 32, 7),        # the widest window the ABI takes
+]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_factored_spmv_and_solve_random_shapes(tl, shape):
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=1000 + npairs, ms=ms,
+                                empty_nodes=0.9 if nnodes > 1000 else 0.1, max_entries=60)
+    rp, ci, va = expand(f)
+    m, n = len(rp) - 1, nnodes * nz
+    S = make(tl, f)
+    assert (S.m, S.n) == (m, n) and S.info("factored") == 1.0 and S.info("lateral_entries") == len(f["lnode"])
+    rng = np.random.default_rng(shape[0])
+    x, u = rng.standard_normal(n), rng.standard_normal(m)
+    for acc, mode, in ((1, oracle.DD), (0, oracle.PLAIN)):
+        S.set(accumulate=acc)
+        y = S.spmv(dev(x)).cpu().numpy()
+        yt = S.spmv(dev(u), transpose=True).cpu().numpy()
+        oy, oyt = oracle.spmv(m, n, rp, ci, va, x, mode), oracle.spmv_t(m, n, rp, ci, va, u, mode)
+        if acc:
+            assert np.array_equal(y, oy) and np.array_equal(yt, oyt)
+        else:
+            scale = np.abs(va).max() * np.abs(x).max()
+            assert np.abs(y - oy).max() <= 1e-12 * scale * 60 * nper * klen
+            assert rel(y, oy) <= 1e-11 and rel(yt, oyt) <= 1e-11   # cancelling random sums: per-row bound above
+    b = rng.standard_normal(m)
+    for solver, ofn in (("lsqr", oracle.lsqr), ("lsmr", oracle.lsmr)):
+        S.set(accumulate=1)
+        xg, res = S.solve(dev(b), damp=0.1, max_iters=20, solver=solver)
+        o = ofn(m, n, rp, ci, va, b, damp=0.1, max_iters=20, mode=oracle.DD)
+        assert res.itn == o.itn and res.istop == o.istop
+        assert np.array_equal(xg.cpu().numpy(), o.x), (solver, rel(xg.cpu().numpy(), o.x))
+    # the CSR path of the library on the multiplied-out matrix gives the same bits
+    C = tl.TomoLsqr(m, n, dev(rp), dev(ci), dev(va))
+    xc, _ = C.solve(dev(b), damp=0.1, max_iters=20)
+    xg, _ = S.solve(dev(b), damp=0.1, max_iters=20)
+    assert torch.equal(xc, xg)
+    C.close(); S.close()
+
+
+def test_factored_cfg0_both_modes(tl, cfg0):
+    s = cfg0["sys"]
+    f = s.factored()
+    m, n, rp, ci, va, b = cfg0["m"], cfg0["n"], cfg0["rp"], cfg0["ci"], cfg0["va"], cfg0["b"]
+    S = make(tl, f)
+    for acc, mode in ((1, oracle.DD), (0, oracle.PLAIN)):
+        S.set(accumulate=acc)
+        xg, res, r2, ar = S.solve(dev(b), damp=s.damp, max_iters=50, history=True)
+        o = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=50, mode=mode)
+        xg = xg.cpu().numpy()
+        assert res.itn == o.itn == 50 and res.istop == o.istop
+        assert rel(xg, o.x) <= TOL_X50
+        assert np.allclose(r2, o.r2norm_hist, rtol=1e-10, atol=0) and np.allclose(ar, o.arnorm_hist, rtol=1e-8, atol=0)
+        for k in ("r1norm", "r2norm", "arnorm", "anorm", "acond", "xnorm"):
+            assert abs(getattr(res, k) - getattr(o, k)) <= 1e-9 * abs(getattr(o, k)), k
+        if acc:
+            assert np.array_equal(xg, o.x) and np.array_equal(r2, o.r2norm_hist)
+    # tolerance stop: same iteration count and reason as the oracle
+    S.set(accumulate=1)
+    xg, res = S.solve(dev(b), damp=s.damp, atol=1e-6, btol=1e-6, max_iters=300)
+    o = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, atol=1e-6, btol=1e-6, max_iters=300, mode=oracle.DD)
+    assert (res.itn, res.istop) == (o.itn, o.istop) and np.array_equal(xg.cpu().numpy(), o.x)
+    # determinism and independence of the launch mode (graph / check_every / pdl), both accumulation modes
+    for acc in (1, 0):
+        S.set(accumulate=acc, graph=1, check_every=10, pdl=1)
+        x1, _ = S.solve(dev(b), damp=s.damp, max_iters=37)
+        x2, _ = S.solve(dev(b), damp=s.damp, max_iters=37)
+        S.set(graph=0, check_every=7, pdl=0)
+        x3, _ = S.solve(dev(b), damp=s.damp, max_iters=37)
+        assert torch.equal(x1, x2) and torch.equal(x1, x3)
+    # host-buffer entry and the sequential multi-RHS entry work on a factored handle
+    S.set(accumulate=1, graph=1, check_every=10, pdl=1)
+    xh = np.empty(n)
+    tl.tomo_lsqr_solve_host(S.h, b, s.damp, 0.0, 0.0, 50, xh)
+    o = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=50, mode=oracle.DD)
+    assert np.array_equal(xh, o.x)
+    B = np.ascontiguousarray(np.stack([b, 2.0 * b[::-1]], axis=1))
+    X, rs = S.solve_multi(dev(B), damp=s.damp, max_iters=50)
+    assert np.array_equal(X[:, 0].cpu().numpy(), o.x)
+    o1 = oracle.lsqr(m, n, rp, ci, va, np.ascontiguousarray(B[:, 1]), damp=s.damp, max_iters=50, mode=oracle.DD)
+    assert np.array_equal(X[:, 1].cpu().numpy(), o1.x)
+    S.close()
+
+
+def test_factored_edge_cases_and_errors(tl):
+    import paper_2604_11920_b200 as T
+    f = tomogen.random_factored(50, 4, 20, 10, 6, seed=77)
+    S = make(tl, f)
+    rp, ci, va = expand(f)
+    m, n = S.m, S.n
+    # b = 0 -> x = 0, istop 0 ; max_iters = 0 -> x = 0, istop 7
+    x, res = S.solve(dev(np.zeros(m)), damp=0.1, max_iters=5)
+    assert res.istop == 0 and res.itn == 0 and not x.any()
+    x, res = S.solve(dev(np.ones(m)), damp=0.1, max_iters=0)
+    assert res.istop == 7 and res.itn == 0 and not x.any()
+    # calls a factored handle does not take
+    for call in (lambda: T.tomo_lsqr_update_values(S.h, dev(va)), lambda: S.csc(), lambda: S.set(compress=1)):
+        with pytest.raises(T.TomoError) as ei:
+            call()
+        assert ei.value.status == T.TOMO_ERR_INVALID_ARG
+    S.close()
+    # malformed operators are rejected at create, *out stays NULL
+    def create(**over):
+        g = dict(f); g.update(over)
+        return make(tl, g)
+    bad_nodes = f["lnode"].copy(); bad_nodes[1] = bad_nodes[0]            # not strictly ascending inside the first pair with >= 2 entries
+    q = int(np.flatnonzero(np.diff(f["lptr"]) >= 2)[0]); bad_nodes = f["lnode"].copy(); bad_nodes[f["lptr"][q] + 1] = bad_nodes[f["lptr"][q]]
+    bad_w = f["lw"].copy(); bad_w[3] = np.inf
+    bad_j0 = f["kj0"].copy(); bad_j0[0] = f["nz"] - f["klen"] + 1
+    bad_kern = f["kern"].copy(); bad_kern[1, 2] = np.nan
+    for over in (dict(lnode=bad_nodes), dict(lw=bad_w), dict(kj0=bad_j0), dict(kern=bad_kern)):
+        with pytest.raises(T.TomoError) as ei:
+            create(**over)
+        assert ei.value.status == T.TOMO_ERR_BAD_CSR, over.keys()
+    with pytest.raises(T.TomoError) as ei:
+        T.tomo_lsqr_create_factored(10, 33, 5, 40, dev(np.zeros(11, dtype=np.int64)), None, None, 4, dev(np.zeros(33, dtype=np.int32)),
+                                    dev(np.zeros(33 * 4)))
+    assert ei.value.status == T.TOMO_ERR_RANGE
+    with pytest.raises(T.TomoError) as ei:   # host pointer
+        T.tomo_lsqr_create_factored(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], dev(f["lnode"]), dev(f["lw"]), f["klen"],
+                                    dev(f["kj0"]), dev(f["kern"]))
+    assert ei.value.status == T.TOMO_ERR_NOT_DEVICE_PTR
+    # a system with no lateral entry at all and one with no extra rows still solve (oracle on the expansion)
+    for g in (tomogen.random_factored(6, 3, 5, 8, 4, seed=5, empty_pairs=1.0), tomogen.random_factored(30, 6, 8, 9, 3, seed=6, ms=0)):
+        rp, ci, va = expand(g)
+        S = make(tl, g)
+        b = np.random.default_rng(1).standard_normal(S.m)
+        x, res = S.solve(dev(b), damp=0.3, max_iters=10)
+        o = oracle.lsqr(S.m, S.n, rp, ci, va, b, damp=0.3, max_iters=10, mode=oracle.DD)
+        assert (res.itn, res.istop) == (o.itn, o.istop) and np.array_equal(x.cpu().numpy(), o.x)
+        S.close()
+
+
+@pytest.fixture(scope="module")
+def big(tl):
+    out = {}
+    for cfg in (1, 4):
+        s = tomogen.System(cfg)
+        out[cfg] = (s, make(tl, s.factored()))
+    return out
+
+
+def test_factored_spmv_cfg1_cfg4(tl, big):
+    for cfg in (1, 4):
+        s, S = big[cfg]
+        d = s.dims
+        rp, ci, va = s.csr()   # = the expansion, bitwise (tests/test_oracle_factored_pins.py)
+        rng = np.random.default_rng(cfg)
+        x, u = rng.standard_normal(d.n), rng.standard_normal(d.m)
+        for acc, mode in ((1, oracle.DD), (0, oracle.PLAIN)):
+            S.set(accumulate=acc)
+            y = S.spmv(dev(x)).cpu().numpy()
+            yt = S.spmv(dev(u), transpose=True).cpu().numpy()
+            oy, oyt = oracle.spmv(d.m, d.n, rp, ci, va, x, mode), oracle.spmv_t(d.m, d.n, rp, ci, va, u, mode)
+            assert rel(y, oy) <= TOL_SPMV and rel(yt, oyt) <= TOL_SPMV
+            if acc:
+                assert np.array_equal(y, oy) and np.array_equal(yt, oyt)
+        assert abs(np.dot(y, u) - np.dot(x, yt)) <= 1e-12 * np.linalg.norm(y) * np.linalg.norm(u)   # adjoint identity
+        del rp, ci, va
+
+
+def test_factored_x50_and_tolerance_run_cfg1(tl, big):
+    s, S = big[1]
+    b = dev(s.rhs(0))
+    o = oracle_jobs.get("cfg1_dd_tol")
+    S.set(accumulate=1)
+    x50, res = S.solve(b, damp=s.damp, max_iters=50)
+    assert rel(x50.cpu().numpy(), o["snapshots"][50]) <= TOL_X50 and np.array_equal(x50.cpu().numpy(), o["snapshots"][50])
+    x, res, r2, ar = S.solve(b, damp=s.damp, atol=1e-6, btol=1e-6, max_iters=300, history=True)
+    assert (res.itn, res.istop) == (o["itn"], o["istop"])
+    assert np.array_equal(x.cpu().numpy(), o["x"]) and np.array_equal(r2, o["r2hist"][: res.itn])
+    # LSMR, the paper's own solver
+    ol = oracle_jobs.get("cfg1_lsmr_dd_50")
+    xl, resl = S.solve(b, damp=s.damp, max_iters=50, solver="lsmr")
+    assert resl.itn == ol["itn"] and np.array_equal(xl.cpu().numpy(), ol["x"])
+    # fast mode: x_10 to the contract, as for the CSR path
+    S.set(accumulate=0)
+    op = oracle_jobs.get("cfg1_plain_50")
+    x10, _ = S.solve(b, damp=s.damp, max_iters=10)
+    assert rel(x10.cpu().numpy(), op["snapshots"][10]) <= TOL_X50
+    S.set(accumulate=1)
+
+
+def test_factored_x50_x100_cfg4_skewed(tl, big):
+    s, S = big[4]
+    b = dev(s.rhs(0))
+    o = oracle_jobs.get("cfg4_dd_100")
+    S.set(accumulate=1)
+    x50, _ = S.solve(b, damp=s.damp, max_iters=50)
+    x100, res = S.solve(b, damp=s.damp, max_iters=100)
+    assert np.array_equal(x50.cpu().numpy(), o["snapshots"][50]) and np.array_equal(x100.cpu().numpy(), o["x"])
+    assert res.itn == o["itn"] == 100
