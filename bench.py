@@ -148,7 +148,8 @@ def workload_config(s, args, iterations_per_step: int, world: int = 1) -> dict:
             "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
             "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
             "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
-            "index": "run-compressed (compress=1)" if args.compress else "int32 per nonzero",
+            "index": ("none: factored operator (lateral footprint x depth kernel, tomo_lsqr_create_factored)" if getattr(args, "factored", 0)
+                      else "run-compressed (compress=1)" if args.compress else "int32 per nonzero"),
             "parallelism": "replicas" if world > 1 else "single GPU",
             "l2": (f"inputs larger than L2: {ab['iteration'] / 1e9:.2f} GB streamed per iteration vs 126 MB L2, no flush needed"
                    if ab["iteration"] > 2 * 126e6 else
@@ -218,16 +219,25 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
     nrhs = s.dims.nrhs
     b_host = torch.from_numpy(s.rhs(0)).pin_memory()
     x_host = torch.empty(n, dtype=torch.float64).pin_memory()
-    rp_d, ci_d, va_d = s.csr_cuda()  # generated and uploaded block by block (config 2: 45 GB)
     vbytes = 8
-    if args.vals == "f32":  # optional fp32 storage of the values (arithmetic stays fp64)
-        va_d, vbytes = va_d.to(torch.float32), 4
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    S = tl.TomoLsqr(m, n, rp_d, ci_d, va_d)
+    factored = bool(getattr(args, "factored", 0))
+    if factored:  # NEXT-2, factored form: lateral footprints + depth kernels + the smoothing block; nothing per nonzero
+        f = s.factored()
+        ft = {k: torch.from_numpy(v).cuda() for k, v in f.items() if hasattr(v, "dtype")}
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        S = tl.TomoLsqr.factored(f["npairs"], f["nper"], f["nnodes"], f["nz"], ft["lptr"], ft["lnode"], ft["lw"], ft["kj0"], ft["kern"],
+                                 ft["sptr"], ft["sidx"], ft["svals"])
+    else:
+        rp_d, ci_d, va_d = s.csr_cuda()  # generated and uploaded block by block (config 2: 45 GB)
+        if args.vals == "f32":  # optional fp32 storage of the values (arithmetic stays fp64)
+            va_d, vbytes = va_d.to(torch.float32), 4
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        S = tl.TomoLsqr(m, n, rp_d, ci_d, va_d)
     torch.cuda.synchronize()
     create_wall_ms = 1e3 * (time.perf_counter() - t0)
-    S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=args.compress)
+    S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=0 if factored else args.compress)
     if args.row_cost is not None:
         S.set(row_cost=args.row_cost)
     if args.pdl is not None:
@@ -280,6 +290,9 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
 
     out = {"m": m, "n": n, "nnz": nnz, "nrhs": nrhs, "vbytes": vbytes, "create_wall_ms": create_wall_ms, "accumulate": args.accumulate,
            "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms")}
+    if factored:
+        out["factored"] = {"lateral_entries": S.info("lateral_entries"), "operator_bytes": S.info("operator_bytes"),
+                           "cut_nodes_pieces": S.info("cut_nodes_pieces")}
     with ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) as clk:
         out["ms"], out["its"], out["launches"] = timed(step_device)
     out["clocks"] = clk.summary()
@@ -298,7 +311,7 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
         ms_o, its_o, _ = timed(step_device)
         out["other"] = {"accumulate": 1 - args.accumulate, "value": its_o / (ms_o * 1e-3), "ms_per_step": ms_o / steps}
         S.set(accumulate=args.accumulate)
-    if args.compress:
+    if args.compress and not factored:
         out["index_bytes"] = (S.info("compress_bytes_rows"), S.info("compress_bytes_cols"))
     S.close()
     return out
@@ -392,6 +405,20 @@ def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
         ab["k1"] += int(r["index_bytes"][0]) - 4 * nnz
         ab["k2"] += int(r["index_bytes"][1]) - 4 * nnz
         note = "run-compressed index (option compress=1): values + measured compressed index bytes + pointers + vectors"
+    if "factored" in r:
+        # The factored operator is L2-resident (operator_bytes per product instead of 12 bytes per nonzero): bound by fp64
+        # arithmetic.  Work per nonzero and product, in fp64 lane-instructions (an FMA counts once): dd 11 = the value
+        # fl(W g) 1 + TwoProd 2 + TwoSum 6 + 2 error adds; fast 2 = the value + the FMA.  Peak as for the dd block solve.
+        per = 11.0 if r.get("accumulate", 1) == 1 else 2.0
+        sm_max = (r.get("clocks") or {}).get("sm_max_mhz") or 1965.0
+        peak_t = 148 * 64 * sm_max * 1e6 / 1e12
+        ach_t = per * nnz * 2 / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e12
+        return {"bound": "alu", "kernel": "k_fac_rows (K1) / k_fac_cols (K2): the two products of an iteration on the factored operator",
+                "achieved": ach_t, "peak": peak_t, "unit": "TFLOP/s", "frac": ach_t / peak_t,
+                "peak_source": "derived: 148 SMs x 64 fp64 lanes/clk x sm_max_mhz (fp64 lane-instructions/s, FMA counted once)",
+                "work_per_launch": per * nnz, "traffic": None, "operator_bytes_per_product": r["factored"]["operator_bytes"],
+                "csr_equivalent_gbs": (ab["k1"] + ab["k2"]) / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e9,
+                "k1_us": r["k1_us"], "k2_us": r["k2_us"], "k4_us": r["k4_us"]}
     spmv_bytes = ab["k1"] + ab["k2"]
     achieved = spmv_bytes / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e9
     kern = ("k_wstream (K1: A v - alpha u + norm over CSR; K2: A^T u - beta v + norm over CSC), mean of the two launches of an iteration"
@@ -454,8 +481,23 @@ def run_ours(args) -> dict | None:
         also["configs[2]"] = {"workload": workload_name(s2), "value": r2["its"] / (r2["ms"] * 1e-3), "unit": UNIT,
                               "accumulate": args.accumulate, "other_mode": r2.get("other"), "ms_per_step": r2["ms"] / 2, "steps": 2,
                               "warmup": 3, "k1_us": r2["k1_us"], "k2_us": r2["k2_us"], "k4_us": r2["k4_us"],
-                              "achieved_gbs": rf2["achieved"], "frac": rf2["frac"], "frac_of_8TBs": rf2["frac_of_8TBs"],
+                              "achieved_gbs": rf2["achieved"] if rf2["bound"] == "hbm" else None, "frac": rf2["frac"], "frac_of_8TBs": rf2.get("frac_of_8TBs"),
+                              "bound": rf2["bound"],
                               "create_ms": r2["create_ms"], "transpose_ms": r2["transpose_ms"], "clocks": r2["clocks"]}
+
+    if world == 1 and args.config == 1 and not args.no_also and not args.factored and args.vals == "f64" and not args.compress:
+        # the same system through the factored operator (NEXT-2, second form): its own line, never mixed into the CSR figures
+        import copy
+        fa = copy.copy(args)
+        fa.factored = 1
+        torch.cuda.empty_cache()
+        rfac = measure(tl, torch, s, fa, barrier, None, 1, args.steps, args.warmup, e2e=False, both_modes=True)
+        rff = roofline_of(rfac, *measured_peak_gbs(), 0)
+        also["configs[1] factored"] = {"workload": workload_name(s), "operator": "factored (tomo_lsqr_create_factored): bitwise the CSR results in dd mode",
+                                       "value": rfac["its"] / (rfac["ms"] * 1e-3), "unit": UNIT, "accumulate": args.accumulate,
+                                       "other_mode": rfac.get("other"), "ms_per_step": rfac["ms"] / args.steps,
+                                       "k1_us": rfac["k1_us"], "k2_us": rfac["k2_us"], "k4_us": rfac["k4_us"], "roofline": rff,
+                                       "create_ms": rfac["create_ms"], "clocks": rfac["clocks"], **rfac["factored"]}
 
     if rank != 0:
         if dist is not None:
@@ -474,7 +516,7 @@ def run_ours(args) -> dict | None:
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": workload_config(s, args, its // max(1, args.steps * world), world),
-        "effective_gbs": eff,
+        "effective_gbs": None if args.factored else eff,  # the factored operator does not move the CSR bytes
         "create_ms": r["create_ms"], "transpose_ms": r["transpose_ms"], "create_wall_ms": r["create_wall_ms"],
         "create_note": "create_ms / transpose_ms: CUDA events inside tomo_lsqr_create (kernels + its cudaMalloc calls); create_wall_ms: host clock around the call",
         "e2e": {"value": r["its_e2e"] / (r["ms_e2e"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * m * nrhs,
@@ -552,6 +594,7 @@ def main():
     ap.add_argument("--solver", default="lsqr", choices=["lsqr", "lsmr"], help="lsqr (BASELINE metric) or lsmr (the paper's solver)")
     ap.add_argument("--vals", default="f64", choices=["f64", "f32"], help="storage type of the matrix values")
     ap.add_argument("--compress", type=int, default=0, choices=[0, 1], help="1: run-compressed index (NEXT-2), reported with its own byte count")
+    ap.add_argument("--factored", type=int, default=0, choices=[0, 1], help="1: the factored operator (NEXT-2, second form), reported against the fp64 pipe")
     ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
     ap.add_argument("--pdl", type=int, default=None, choices=[0, 1], help="tuning: programmatic dependent launch between the kernels of an iteration")
     ap.add_argument("--shards", type=int, default=0, help="NEXT-3: P row blocks solved by tomo_lsqr_solve_sharded (one GPU: all blocks local; torchrun: one block per rank)")

@@ -50,6 +50,7 @@ struct FacDesc {       // uniform kernel argument
   const FacSeg* seg;
   double2* seg_part;       // unrounded partial layer sums of the pieces of cut nodes
   unsigned int* node_cnt;  // arrivals per cut node; zero between launches
+  long long* busy;         // per warp: cycles of its share of the most recent product launch (load balance read-out)
   double2* node_nsq;       // per node: sum of the squares of its nz results (unrounded pair), summed in node order by the last CTA
 };
 
@@ -108,6 +109,7 @@ k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
   const int64_t x0 = d.ms * gw / NW, x1 = d.ms * (int64_t)(gw + 1) / NW;  // this warp's share of the extra rows
 
   grid_dependency_wait();
+  const long long t_start = clock64();
   double c = 0.0, sy = 1.0;
   if (K1) {
     if (sc->stop) return;
@@ -161,6 +163,7 @@ k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
     const double yo = K1 ? y[ro] * sy : 0.0;
     y[ro] = fac_finish<MODE, K1, K1>(a, c, yo, nsq);
   }
+  if (lane == 0) d.busy[gw] = clock64() - t_start;
   if (!K1) return;
 
   lanes_reduce<32, MODE>(nsq);
@@ -216,13 +219,60 @@ k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
     if (OP == OP_K2) c = -sc->beta;
     sx = sc->rbeta;
   }
+  const long long t_start = clock64();
 
+  FacSeg sg_next = {};
+  if (s0 < s1) sg_next = d.seg[s0];
   for (int s = s0; s < s1; ++s) {
-    const FacSeg sg = d.seg[s];
+    const FacSeg sg = sg_next;
+    if (s + 1 < s1) sg_next = d.seg[s + 1];   // the next piece's descriptor is on its way
+    // the range of the extra block's column this lane will close (layer = lane): on its way during the sums
+    int64_t xc0 = 0, xc1 = 0;
+    if (d.scptr && lane < nz) { const int64_t colp = (int64_t)sg.node * nz + lane; xc0 = d.scptr[colp]; xc1 = d.scptr[colp + 1]; }
     Acc<MODE> acc[KLP];
 #pragma unroll
     for (int t = 0; t < KLP; ++t) acc[t].zero();
-    if (active) {
+    // The piece's entries go by in batches of SB steps (SB * G <= 32 entries): lane l loads entry l of the batch
+    // (coalesced, one batch ahead), the lanes of group g pick entry step * G + g up by shuffle, and the gathers of U
+    // steps are in flight before their sums start (the pair number no longer sits between two dependent loads).
+    if (MODE == 0) {
+      constexpr int U = 5;
+      const int SB = 32 / G, BE = SB * G;
+      int64_t eb = sg.e0;
+      int qreg = 0;
+      double wreg = 0.0;
+      if (lane < BE && eb + lane < sg.e1) { qreg = d.cpair[eb + lane]; wreg = d.cw[eb + lane]; }
+      while (eb < sg.e1) {
+        const int nb = (int)((sg.e1 - eb < (int64_t)BE) ? (sg.e1 - eb) : (int64_t)BE);
+        const int64_t en = eb + BE;
+        int qn = 0;
+        double wn = 0.0;
+        if (lane < BE && en + lane < sg.e1) { qn = d.cpair[en + lane]; wn = d.cw[en + lane]; }
+        for (int st = 0; st * G < nb; st += U) {
+          double xs[U], ws[U];
+          bool ok[U];
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int src = (st + u) * G + g;
+            ok[u] = active && src < nb;
+            const int q = __shfl_sync(0xffffffffu, qreg, src & 31);
+            ws[u] = __shfl_sync(0xffffffffu, wreg, src & 31);
+            xs[u] = ok[u] ? x[(int64_t)q * nper + p] : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            if (ok[u]) {
+              const double us = SCALE ? xs[u] * sx : xs[u];
+#pragma unroll
+              for (int t = 0; t < KLP; ++t)
+                if (!GUARD || t < klen) acc[t].mac(ws[u] * kr[t], us);
+            }
+          }
+        }
+        qreg = qn; wreg = wn; eb = en;
+      }
+    } else if (active) {
+      // dd mode: 11 fp64 instructions per product keep the pipe busy; one entry ahead is enough
       int64_t e = sg.e0 + g;
       bool has = e < sg.e1;
       int q = has ? d.cpair[e] : 0;
@@ -239,8 +289,11 @@ k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
           if (!GUARD || t < klen) acc[t].mac(wc * kr[t], us);
       }
     }
+    const bool none = sg.e0 == sg.e1;   // a node no ray touches: closed from the extra block alone
+    if (!none) {
 #pragma unroll
-    for (int t = 0; t < KLP; ++t) my[t * 32 + lane] = acc[t].pack();
+      for (int t = 0; t < KLP; ++t) my[t * 32 + lane] = acc[t].pack();
+    }
     __syncwarp();
     const int node = sg.node;
     const bool whole = sg.nsegs == 1;
@@ -249,22 +302,36 @@ k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
     // the closing of layer j of this node: the extra rows' column, the axpy, the rounding, the norm
     auto close = [&](int j, Acc<MODE> S) {
       const int64_t col = (int64_t)node * nz + j;
-      if (d.scptr) {
-        for (int64_t e = d.scptr[col]; e < d.scptr[col + 1]; ++e) {
-          const double xe = x[d.mdata + d.srow[e]];
-          S.mac(d.scval[e], SCALE ? xe * sx : xe);
+      const double yo = AXPY ? y[col] : 0.0;
+      if (d.scptr) {   // eight entries at a time: the loads of one level are all in flight before the next level starts
+        const int64_t c0 = (j == lane) ? xc0 : d.scptr[col], c1 = (j == lane) ? xc1 : d.scptr[col + 1];
+        for (int64_t base = c0; base < c1; base += 8) {
+          int32_t rr[8];
+          double vv[8], xe[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const bool in = base + i < c1;
+            rr[i] = in ? d.srow[base + i] : 0;
+            vv[i] = in ? d.scval[base + i] : 0.0;
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) xe[i] = (base + i < c1) ? x[d.mdata + rr[i]] : 0.0;
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            if (base + i < c1) S.mac(vv[i], SCALE ? xe[i] * sx : xe[i]);
         }
       }
-      const double yo = AXPY ? y[col] : 0.0;
       y[col] = fac_finish<MODE, AXPY, NORM>(S, c, yo, nsq);
     };
     for (int j = lane; j < nz; j += 32) {   // layer sums over periods (ascending) and groups (ascending): fixed order
       Acc<MODE> S;
       S.zero();
-      for (int pp = 0; pp < nper; ++pp) {
-        const int t = j - s_kj0[pp];
-        if (t >= 0 && t < klen)
-          for (int gg = 0; gg < G; ++gg) S.merge(fac_acc_of<MODE>(my[t * 32 + gg * nper + pp]));
+      if (!none) {
+        for (int pp = 0; pp < nper; ++pp) {
+          const int t = j - s_kj0[pp];
+          if (t >= 0 && t < klen)
+            for (int gg = 0; gg < G; ++gg) S.merge(fac_acc_of<MODE>(my[t * 32 + gg * nper + pp]));
+        }
       }
       if (whole) close(j, S);
       else __stcg(d.seg_part + (size_t)sg.slot * nz + j, S.pack());
@@ -290,12 +357,14 @@ k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
     }
     if (NORM && closer) {
       lanes_reduce<32, MODE>(nsq);
-      if (lane == 0) { __stcg(d.node_nsq + node, nsq.pack()); __threadfence(); }
+      if (lane == 0) __stcg(d.node_nsq + node, nsq.pack());
     }
     __syncwarp();
   }
+  if (lane == 0) d.busy[gw] = clock64() - t_start;
   if (!NORM) return;
 
+  __threadfence();   // the per-node norm pairs this warp wrote, before the CTA takes its ticket
   __syncthreads();
   grid_launch_dependents();
   if (!fac_ticket(sc, &s_flag)) return;

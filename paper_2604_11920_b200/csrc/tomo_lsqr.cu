@@ -71,14 +71,15 @@ struct Dir {
 // the factored sensitivity block (factored.cuh; tomo_lsqr_create_factored): what the handle owns of it
 struct FacState {
   FacDesc d = {};                 // the kernel argument (borrowed W / A_extra CSR arrays, owned rest)
+  FacDesc dm[2];                  // ... per accumulation mode: the A^T x work split differs (wseg, seg)
   int64_t E = 0, snnz = 0;        // lateral entries, entries of the extra rows
   int klp = 0; bool guard = false;  // kernel shape: window length as a template constant (8, 12, 16) or the general one (32, guarded)
   int nsegs = 0, nslots = 0;
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
-  int32_t* pw = nullptr; int32_t* wseg = nullptr; FacSeg* seg = nullptr;
-  double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr;
+  int32_t* pw = nullptr; int32_t* wseg[2] = {nullptr, nullptr}; FacSeg* seg[2] = {nullptr, nullptr};
+  double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
 };
 
 struct tomo_lsqr_s {
@@ -226,12 +227,12 @@ cudaError_t launch_fac_one(const tomo_lsqr_s* h, bool cols, const double* x, dou
   if (cols) {
     if constexpr (OP == OP_PLAIN || OP == OP_K2 || OP == OP_K2_INIT) {
       cfg.dynamicSmemBytes = fac_cols_smem<KLP, GUARD>();
-      return cudaLaunchKernelEx(&cfg, k_fac_cols<MODE, OP, KLP, GUARD>, h->fac->d, x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac_cols<MODE, OP, KLP, GUARD>, h->fac->dm[MODE], x, y, h->sc, h->part_spmv);
     }
   } else {
     if constexpr (OP == OP_PLAIN || OP == OP_K1) {
       cfg.dynamicSmemBytes = 0;
-      return cudaLaunchKernelEx(&cfg, k_fac_rows<MODE, OP, KLP, GUARD>, h->fac->d, x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac_rows<MODE, OP, KLP, GUARD>, h->fac->dm[MODE], x, y, h->sc, h->part_spmv);
     }
   }
   return cudaErrorInvalidValue;
@@ -470,8 +471,8 @@ void free_handle(tomo_lsqr_s* h) {
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
     cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
-    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->wseg); cudaFree(f->seg);
-    cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq);
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); for (int i = 0; i < 2; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
+    cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
   }
   cudaFree(h->cta_rec);
@@ -661,9 +662,10 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     const int G = 32 / nper;
     std::vector<int32_t> pw((size_t)NW + 1);
     {
-      // cost of a pair in lane steps: ceil(entries / G) + 4 (group combine, row stores)
+      // cost of a pair in lane steps: ceil(entries / G) + 0.3 (group combine, row stores; fitted to the per-warp busy
+      // cycles on B200: 245 cycles per pair against 918 per step in dd mode, 104 against 512 in fast mode)
       std::vector<double> pre((size_t)npairs + 1, 0.0);
-      for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 4.0;
+      for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 0.3;
       int64_t q = 0;
       pw[0] = 0;
       for (int w = 1; w < NW; ++w) {
@@ -676,26 +678,50 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     std::vector<int64_t> cptr((size_t)nnodes + 1);
     if ((e = cudaMemcpyAsync(cptr.data(), f->cptr, sizeof(int64_t) * (nnodes + 1), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the node pointers"); break; }
-    std::vector<FacSeg> segs;
-    std::vector<int32_t> wseg((size_t)NW + 1, 0), owner;
-    {
-      auto bound = [&](int w) { return (int64_t)((double)E * (double)w / (double)NW); };   // first entry of warp w's range
+    std::vector<FacSeg> segs_m[2];
+    std::vector<int32_t> wseg_m[2];
+    int nslots_max = 0;
+    for (int mode = 0; mode < 2; ++mode) {
+      std::vector<FacSeg>& segs = segs_m[mode];
+      std::vector<int32_t>& wseg = wseg_m[mode];
+      std::vector<int32_t> owner;
+      wseg.assign((size_t)NW + 1, 0);
+      // Cost axis: a node costs a closing overhead (in entry units: the layer sums through shared memory, the extra
+      // block's column, the stores) followed by one unit per entry; the warps own equal stretches of that axis.  A
+      // node whose entries straddle a boundary is cut there (pieces of at least kMinPiece entries).
+      // measured on B200 (per-warp busy cycles): closing a node is a chain of dependent loads worth ~5 k cycles,
+      // i.e. the time of ~26 entries in dd mode and ~55 in fast mode, hence one split per mode
+      const double kClose = mode ? 26.0 : 55.0, kCloseEmpty = mode ? 14.0 : 28.0;
+      const int64_t kMinPiece = 8;
+      int64_t empty = 0;
+      for (int64_t k = 0; k < nnodes; ++k) empty += cptr[k] == cptr[k + 1];
+      const double C = (double)E + kClose * (double)(nnodes - empty) + kCloseEmpty * (double)empty;
+      auto bound = [&](int w) { return C * (double)w / (double)NW; };   // start of warp w's stretch
       int w = 0, nslots = 0;
+      double cum = 0.0;
       for (int64_t k = 0; k < nnodes; ++k) {
         const int64_t lo = cptr[k], hi = cptr[k + 1];
         const size_t first = segs.size();
+        while (w + 1 < NW && bound(w + 1) <= cum) ++w;
         if (lo == hi) {
-          if (E == 0) w = (int)(k * NW / nnodes);
-          else while (w + 1 < NW && bound(w + 1) <= lo) ++w;
           segs.push_back(FacSeg{lo, lo, (int32_t)k, 1, 0, 0}); owner.push_back(w);
+          cum += kCloseEmpty;
         } else {
+          const double ent0 = cum + kClose;   // cost position of the node's first entry
           int64_t a = lo;
           while (a < hi) {
-            while (w + 1 < NW && bound(w + 1) <= a) ++w;
-            const int64_t b = (w + 1 < NW) ? std::min(hi, std::max(bound(w + 1), a + 1)) : hi;
-            segs.push_back(FacSeg{a, b, (int32_t)k, 1, 0, 0}); owner.push_back(w);
-            a = b;
+            int64_t b2 = hi;
+            if (w + 1 < NW) {
+              const double room = bound(w + 1) - ent0;   // entries of this node that fit before the boundary
+              int64_t lim = lo + (room > 0.0 ? (int64_t)room : 0);
+              lim = std::max(lim, a + std::min<int64_t>(kMinPiece, hi - a));
+              b2 = (hi - lim < kMinPiece) ? hi : std::min(lim, hi);
+            }
+            segs.push_back(FacSeg{a, b2, (int32_t)k, 1, 0, 0}); owner.push_back(w);
+            a = b2;
+            if (a < hi) { const double pos = ent0 + (double)(a - lo); while (w + 1 < NW && bound(w + 1) <= pos) ++w; }
           }
+          cum = ent0 + (double)(hi - lo);
         }
         const int cnt = (int)(segs.size() - first);
         if (cnt > 1) {
@@ -706,14 +732,22 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       for (size_t i = 0; i < segs.size(); ++i) wseg[(size_t)owner[i] + 1] += 1;
       for (int i = 0; i < NW; ++i) wseg[i + 1] += wseg[i];
       f->nsegs = (int)segs.size(); f->nslots = nslots;
+      nslots_max = std::max(nslots_max, nslots);
     }
-    ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->wseg, sizeof(int32_t) * (NW + 1));
-    ALLOC(f->seg, sizeof(FacSeg) * std::max<size_t>(segs.size(), 1));
-    ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(f->nslots, 1) * nz);
+    ALLOC(f->pw, sizeof(int32_t) * (NW + 1));
+    for (int mode = 0; mode < 2 && rc == TOMO_OK; ++mode) {
+      if ((e = cudaMalloc(&f->wseg[mode], sizeof(int32_t) * (NW + 1))) != cudaSuccess ||
+          (e = cudaMalloc(&f->seg[mode], sizeof(FacSeg) * std::max<size_t>(segs_m[mode].size(), 1))) != cudaSuccess ||
+          (e = cudaMemcpyAsync(f->wseg[mode], wseg_m[mode].data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(f->seg[mode], segs_m[mode].data(), sizeof(FacSeg) * segs_m[mode].size(), cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        rc = cuda_fail(e, "upload of the A^T x work split");
+    }
+    if (rc != TOMO_OK) break;
+    ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(nslots_max, 1) * nz);
     ALLOC(f->node_cnt, sizeof(unsigned int) * nnodes); ALLOC(f->node_nsq, sizeof(double2) * nnodes);
+    ALLOC(f->busy, sizeof(long long) * NW);
+    if ((e = cudaMemsetAsync(f->busy, 0, sizeof(long long) * NW, st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
     if ((e = cudaMemcpyAsync(f->pw, pw.data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(f->wseg, wseg.data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(f->seg, segs.data(), sizeof(FacSeg) * segs.size(), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemsetAsync(f->node_cnt, 0, sizeof(unsigned int) * nnodes, st)) != cudaSuccess ||
         (e = cudaMemsetAsync(f->node_nsq, 0, sizeof(double2) * nnodes, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the work split"); break; }
@@ -740,8 +774,9 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     d.kj0 = f->kj0; d.kern = f->kern;
     d.sptr = d_sptr; d.sidx = d_sidx; d.sval = d_svals;
     d.scptr = f->scptr; d.srow = f->srow; d.scval = f->scval;
-    d.pw = f->pw; d.wseg = f->wseg; d.seg = f->seg;
-    d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq;
+    d.pw = f->pw; d.wseg = f->wseg[1]; d.seg = f->seg[1];
+    d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq; d.busy = f->busy;
+    for (int mode = 0; mode < 2; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
     cudaEventRecord(e1, st);
     if ((e = cudaEventSynchronize(e1)) != cudaSuccess) { rc = cuda_fail(e, "create_factored"); break; }
     float msf = 0;
@@ -1436,6 +1471,22 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   else if (k == "operator_bytes")   // what a product has to read of the operator itself
     *out = h->fac ? 12.0 * (double)h->fac->E + 8.0 * (double)(h->fac->d.npairs + 1) + 12.0 * (double)h->fac->snnz + 8.0 * (double)(h->fac->d.ms + 1)
                   : (double)h->nnz * (4.0 + vb) + 8.0 * (double)(h->m + 1);
+  else if (h->fac && (k == "warp_busy_min" || k == "warp_busy_mean" || k == "warp_busy_max" || k == "warp_busy_argmax")) {
+    // busy cycles of the warps in the most recent product launch on the factored operator (balance of the static split)
+    const int NW = h->sms * kFacWarps;
+    std::vector<long long> b((size_t)NW);
+    CK(cudaMemcpy(b.data(), h->fac->busy, sizeof(long long) * NW, cudaMemcpyDeviceToHost));
+    double mn = 1e300, mx = -1, sum = 0; int arg = 0;
+    for (int i = 0; i < NW; ++i) { const double c = (double)b[i]; mn = std::min(mn, c); if (c > mx) { mx = c; arg = i; } sum += c; }
+    *out = k == "warp_busy_min" ? mn : k == "warp_busy_max" ? mx : k == "warp_busy_argmax" ? (double)arg : sum / NW;
+  }
+  else if (h->fac && k.rfind("warp_busy@", 0) == 0) {   // one warp's figure
+    const int i = atoi(k.c_str() + 10);
+    if (i < 0 || i >= h->sms * kFacWarps) return TOMO_ERR_INVALID_ARG;
+    long long b = 0;
+    CK(cudaMemcpy(&b, h->fac->busy + i, sizeof(long long), cudaMemcpyDeviceToHost));
+    *out = (double)b;
+  }
   else if (h->fac && (k == "csc_bytes" || k.rfind("compress_bytes", 0) == 0 || k.rfind("cta_busy", 0) == 0)) return TOMO_ERR_INVALID_ARG;
   else if (k == "transpose_ms") *out = h->transpose_ms;
   else if (k == "transpose_kernels_ms") *out = h->transpose_kernels_ms;
