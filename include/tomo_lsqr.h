@@ -211,7 +211,11 @@ tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, int64_t value
  * the A v, A^T u and vector kernels over the iterations that ran) and "k_launches" (launches of each);
  * "kernels_enqueued": cumulative number of kernel launches this handle has issued in solves (nodes of
  * replayed graphs included); "cta_busy_min" / "cta_busy_mean" / "cta_busy_max": busy cycles of the persistent
- * CTAs in the most recent sparse-product launch (load balance of the static split). */
+ * CTAs in the most recent sparse-product launch (load balance of the static split).  Every handle: "factored" (0 | 1),
+ * "operator_bytes" (what one product reads of the operator itself).  Factored handles only: "lateral_entries",
+ * "cut_nodes_pieces" (pieces of the nodes the A^T x split cuts, current accumulation mode's split counted last),
+ * "warp_busy_min" / "_mean" / "_max" / "_argmax" and "warp_busy@<i>" (busy cycles of the warps in the most recent
+ * product launch); "csc_bytes", "compress_bytes_*" and "cta_busy_*" are INVALID_ARG on a factored handle. */
 tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, double* out);
 
 /* The sparse product for callers that cannot allocate (code under CUDA graph capture, tight serving loops,

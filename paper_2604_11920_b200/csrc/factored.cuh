@@ -45,7 +45,8 @@ struct FacDesc {       // uniform kernel argument
   const int32_t* kj0; const double* kern;                            // [nper], [nper * klen]
   const int64_t* sptr; const int32_t* sidx; const double* sval;      // A_extra as CSR (ms x n); NULL if ms == 0
   const int64_t* scptr; const int32_t* srow; const double* scval;    // A_extra as CSC; NULL if it has no entries
-  const int32_t* pw;       // k_fac_rows: first pair of every warp [NW + 1]
+  const int32_t* pw;       // k_fac_rows: warp w walks the pairs pq[pw[w]] .. pq[pw[w + 1] - 1] (ascending)
+  const int32_t* pq;
   const int32_t* wseg;     // k_fac_cols: first piece of every warp [NW + 1]
   const FacSeg* seg;
   double2* seg_part;       // unrounded partial layer sums of the pieces of cut nodes
@@ -105,6 +106,9 @@ k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
 #pragma unroll
   for (int t = 0; t < KLP; ++t) kr[t] = (!GUARD || t < klen) ? d.kern[(size_t)p * klen + t] : 0.0;
   const int j0 = d.kj0[p];
+  constexpr bool VEC2 = (MODE == 0) && !GUARD && (KLP % 2 == 0);
+  const bool vec2 = ((d.nz & 1) == 0) && ((reinterpret_cast<uintptr_t>(x) & 15u) == 0);   // pairs of layers are 16-byte aligned
+  const int jodd = j0 & 1;
   const int q0 = d.pw[gw], q1 = d.pw[gw + 1];
   const int64_t x0 = d.ms * gw / NW, x1 = d.ms * (int64_t)(gw + 1) / NW;  // this warp's share of the extra rows
 
@@ -118,7 +122,10 @@ k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
   Acc<MODE> nsq;
   nsq.zero();
 
-  for (int q = q0; q < q1; ++q) {
+  int q_next = (q0 < q1) ? d.pq[q0] : 0;
+  for (int i = q0; i < q1; ++i) {
+    const int q = q_next;
+    if (i + 1 < q1) q_next = d.pq[i + 1];
     const int64_t e0 = d.lptr[q], e1 = d.lptr[q + 1];
     Acc<MODE> a0, a1;
     a0.zero(); a1.zero();
@@ -130,8 +137,20 @@ k_fac_rows(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
       while (has) {
         const double* xp = x + (int64_t)k * d.nz + j0;
         double xv[KLP];
+        if (VEC2 && vec2) {
+          // fast mode is bound by L1 wavefronts (one 8-byte gather per product): fetch the window as 16-byte pairs
+          // from the even layer at or below j0_p and pick the lane's klen values out of them
+          const double2* xq = reinterpret_cast<const double2*>(xp - jodd);
+          double fl[KLP + 2];
 #pragma unroll
-        for (int t = 0; t < KLP; ++t) xv[t] = (!GUARD || t < klen) ? xp[t] : 0.0;
+          for (int i = 0; i < KLP / 2; ++i) { const double2 v2 = xq[i]; fl[2 * i] = v2.x; fl[2 * i + 1] = v2.y; }
+          fl[KLP] = jodd ? xp[KLP - 1] : 0.0;   // an odd window ends one layer past the last pair
+#pragma unroll
+          for (int t = 0; t < KLP; ++t) xv[t] = jodd ? fl[t + 1] : fl[t];
+        } else {
+#pragma unroll
+          for (int t = 0; t < KLP; ++t) xv[t] = (!GUARD || t < klen) ? xp[t] : 0.0;
+        }
         const double wc = w;
         e += G;
         has = e < e1;

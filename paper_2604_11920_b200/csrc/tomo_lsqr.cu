@@ -78,7 +78,7 @@ struct FacState {
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
-  int32_t* pw = nullptr; int32_t* wseg[2] = {nullptr, nullptr}; FacSeg* seg[2] = {nullptr, nullptr};
+  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[2] = {nullptr, nullptr}; FacSeg* seg[2] = {nullptr, nullptr};
   double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
 };
 
@@ -471,7 +471,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
     cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
-    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); for (int i = 0; i < 2; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); for (int i = 0; i < 2; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
     cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
   }
@@ -660,20 +660,45 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
         (e = cudaMemcpyAsync(f->kern, d_kern, sizeof(double) * nper * klen, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the kernel table"); break; }
     // --- static work split (host): pairs by entry count for A x; lateral-CSC entries cut evenly for A^T x ---
     const int G = 32 / nper;
-    std::vector<int32_t> pw((size_t)NW + 1);
+    std::vector<int32_t> pw((size_t)NW + 1), pq((size_t)npairs);
     {
       // cost of a pair in lane steps: ceil(entries / G) + 0.3 (group combine, row stores; fitted to the per-warp busy
-      // cycles on B200: 245 cycles per pair against 918 per step in dd mode, 104 against 512 in fast mode)
+      // cycles on B200: 245 cycles per pair against 918 per step in dd mode, 104 against 512 in fast mode).
+      // A CTA takes a contiguous run of pairs (equal cost); inside the CTA the pairs are dealt to the warps longest
+      // first, each to the least loaded warp (a contiguous split at pair granularity left +-18 % between warps);
+      // a warp walks its pairs in ascending order.
+      auto cost = [&](int64_t q) { return (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 0.3; };
       std::vector<double> pre((size_t)npairs + 1, 0.0);
-      for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 0.3;
+      for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + cost(q);
+      std::vector<int64_t> pc((size_t)sms + 1, 0);
       int64_t q = 0;
-      pw[0] = 0;
-      for (int w = 1; w < NW; ++w) {
-        const double target = pre[npairs] * (double)w / (double)NW;
+      for (int c = 1; c < sms; ++c) {
+        const double target = pre[npairs] * (double)c / (double)sms;
         while (q < npairs && 0.5 * (pre[q] + pre[q + 1]) < target) ++q;
-        pw[w] = (int32_t)q;
+        pc[c] = q;
       }
-      pw[NW] = (int32_t)npairs;
+      pc[sms] = npairs;
+      std::vector<int64_t> items;
+      std::vector<std::vector<int32_t>> bins(kFacWarps);
+      size_t outp = 0;
+      for (int c = 0; c < sms; ++c) {
+        items.clear();
+        for (int64_t i = pc[c]; i < pc[c + 1]; ++i) items.push_back(i);
+        std::stable_sort(items.begin(), items.end(), [&](int64_t a2, int64_t b2) { return cost(a2) > cost(b2); });
+        double load[kFacWarps] = {};
+        for (auto& bn : bins) bn.clear();
+        for (int64_t i : items) {
+          int best = 0;
+          for (int w = 1; w < kFacWarps; ++w) if (load[w] < load[best]) best = w;
+          bins[best].push_back((int32_t)i); load[best] += cost(i);
+        }
+        for (int w = 0; w < kFacWarps; ++w) {
+          std::sort(bins[w].begin(), bins[w].end());
+          pw[(size_t)c * kFacWarps + w] = (int32_t)outp;
+          for (int32_t i : bins[w]) pq[outp++] = i;
+        }
+      }
+      pw[NW] = (int32_t)outp;
     }
     std::vector<int64_t> cptr((size_t)nnodes + 1);
     if ((e = cudaMemcpyAsync(cptr.data(), f->cptr, sizeof(int64_t) * (nnodes + 1), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
@@ -734,7 +759,8 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       f->nsegs = (int)segs.size(); f->nslots = nslots;
       nslots_max = std::max(nslots_max, nslots);
     }
-    ALLOC(f->pw, sizeof(int32_t) * (NW + 1));
+    ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->pq, sizeof(int32_t) * npairs);
+    if ((e = cudaMemcpyAsync(f->pq, pq.data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the pair lists"); break; }
     for (int mode = 0; mode < 2 && rc == TOMO_OK; ++mode) {
       if ((e = cudaMalloc(&f->wseg[mode], sizeof(int32_t) * (NW + 1))) != cudaSuccess ||
           (e = cudaMalloc(&f->seg[mode], sizeof(FacSeg) * std::max<size_t>(segs_m[mode].size(), 1))) != cudaSuccess ||
@@ -774,7 +800,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     d.kj0 = f->kj0; d.kern = f->kern;
     d.sptr = d_sptr; d.sidx = d_sidx; d.sval = d_svals;
     d.scptr = f->scptr; d.srow = f->srow; d.scval = f->scval;
-    d.pw = f->pw; d.wseg = f->wseg[1]; d.seg = f->seg[1];
+    d.pw = f->pw; d.pq = f->pq; d.wseg = f->wseg[1]; d.seg = f->seg[1];
     d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq; d.busy = f->busy;
     for (int mode = 0; mode < 2; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
     cudaEventRecord(e1, st);
