@@ -249,3 +249,41 @@ def test_factored_x50_x100_cfg4_skewed(tl, big):
     x100, res = S.solve(b, damp=s.damp, max_iters=100)
     assert np.array_equal(x50.cpu().numpy(), o["snapshots"][50]) and np.array_equal(x100.cpu().numpy(), o["x"])
     assert res.itn == o["itn"] == 100
+
+
+def test_factored_cfg2_full_size(tl):
+    """configs[2] (3.7e9 nonzeros as CSR; 236 MB factored): sampled rows of A x and sampled columns' worth of A^T x
+    against the oracle on the generator's rows, and x_1, x_2, x_5 bitwise against the dd oracle's full-size run (the
+    background job of test_gpu_parity.py; its matrix is the generator's CSR = the multiplied-out operator)."""
+    s = tomogen.System(2)
+    d = s.dims
+    S = make(tl, s.factored())
+    assert (S.m, S.n) == (d.m, d.n)
+    rng = np.random.default_rng(2)
+    x = rng.standard_normal(d.n)
+    rows = np.unique(np.concatenate([[0, d.m_data - 1, d.m_data, d.m - 1], rng.integers(0, d.m, size=2000)]))
+    rp, ci, va = s.rows(rows)
+    for acc, mode in ((1, oracle.DD), (0, oracle.PLAIN)):
+        S.set(accumulate=acc)
+        y = S.spmv(dev(x)).cpu().numpy()[rows]
+        oy = oracle.spmv(len(rows), d.n, rp, ci, va, x, mode)
+        assert rel(y, oy) <= TOL_SPMV
+        if acc:
+            assert np.array_equal(y, oy)
+    # A^T: adjoint identity with the product just checked (every column enters)
+    S.set(accumulate=1)
+    u = rng.standard_normal(d.m)
+    yt = S.spmv(dev(u), transpose=True).cpu().numpy()
+    yx = S.spmv(dev(x)).cpu().numpy()
+    assert abs(np.dot(yx, u) - np.dot(x, yt)) <= 1e-12 * np.linalg.norm(yx) * np.linalg.norm(u)
+    b = dev(s.rhs(0))
+    xk = {k: S.solve(b, damp=s.damp, max_iters=k)[0].cpu().numpy() for k in (1, 2, 5)}
+    x100a, res = S.solve(b, damp=s.damp, max_iters=100)
+    x100b, _ = S.solve(b, damp=s.damp, max_iters=100)
+    assert res.itn == 100 and torch.equal(x100a, x100b)
+    S.close()
+    o = oracle_jobs.get("cfg2_dd_5")
+    if "skipped" in o:
+        pytest.skip("config-2 x_k parity of the factored operator not run: " + o["skipped"])
+    for k, want in ((1, o["snapshots"][1]), (2, o["snapshots"][2]), (5, o["x"])):
+        assert rel(xk[k], want) <= TOL_X50 and np.array_equal(xk[k], want), k
