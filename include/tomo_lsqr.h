@@ -106,6 +106,21 @@ tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npairs, int32_
                                         const int64_t* d_sptr, const int32_t* d_sidx, const double* d_svals,
                                         void* cuda_stream);
 
+/* NEXT-4 ("on-device assembly of G from ray paths and depth kernels"; Eq. 5, Eq. 7):
+ * multiply the factored description (arguments as tomo_lsqr_create_factored) out into the canonical CSR arrays the general
+ * path takes, on the device: d_rowptr int64[m + 1], d_colind int32[nnz], d_vals fp64[nnz], caller-allocated DEVICE arrays,
+ * fully overwritten; nnz must equal d_lptr[npairs] * nper * klen + snnz (INVALID_ARG otherwise, nothing written).
+ * Row q * nper + p holds, for the pair's lateral entries in order, value fl(W[q, k] * g_p[t]) at column k * nz + j0_p + t
+ * (t = 0 .. klen - 1); the extra block follows unchanged.  The inputs are NOT validated here (tomo_lsqr_create on the
+ * result validates the matrix).  One HBM-bound pass: 12 bytes written per nonzero.  The outer Gauss-Newton loop
+ * re-evaluates the depth kernels every iteration: this call (or tomo_lsqr_create_factored, which needs no assembly at all)
+ * replaces the host-side assembly.  Errors: INVALID_ARG, RANGE, NOT_DEVICE_PTR, UNSUPPORTED_ARCH, CUDA. */
+tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz, const int64_t* d_lptr,
+                                     const int32_t* d_lnode, const double* d_lw, int32_t klen, const int32_t* d_kj0,
+                                     const double* d_kern, int64_t ms, int64_t snnz, const int64_t* d_sptr, const int32_t* d_sidx,
+                                     const double* d_svals, int64_t nnz, int64_t* d_rowptr, int32_t* d_colind, double* d_vals,
+                                     void* cuda_stream);
+
 /* NEXT-4: value-only refresh.  The outer Gauss-Newton loop of the inversion
  * re-evaluates G on the same rays and solves again: the sparsity pattern, hence the CSC permutation, the split
  * points and the compressed index, stay; only the values change.  d_vals: device array [nnz] of the handle's value

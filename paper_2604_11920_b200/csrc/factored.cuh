@@ -49,7 +49,8 @@ struct FacDesc {       // uniform kernel argument
   const int32_t* pq;
   const int32_t* wseg;     // k_fac_cols: first piece of every warp [NW + 1]
   const FacSeg* seg;
-  double2* seg_part;       // unrounded partial layer sums of the pieces of cut nodes
+  double2* seg_part;       // unrounded partial layer sums of the pieces of cut nodes (slot stride nz; two-stage: pstride)
+  int64_t pstride;         // max(nz, nper): slot stride of the two-stage kernels (they publish nper values per piece)
   unsigned int* node_cnt;  // arrivals per cut node; zero between launches
   long long* busy;         // per warp: cycles of its share of the most recent product launch (load balance read-out)
   double2* node_nsq;       // per node: sum of the squares of its nz results (unrounded pair), summed in node order by the last CTA
@@ -404,6 +405,307 @@ __global__ void k_fac_validate_kern(int nper, int nz, int klen, const int32_t* _
   for (int i = threadIdx.x; i < nper * klen; i += blockDim.x)
     if (!(fabs(kern[i]) <= 1.79769313486231570815e308)) bad = 1;
   if (bad) atomicOr(flags, 1);
+}
+
+}  // namespace tomo
+
+namespace tomo {
+
+// ------------------------------------------------------------------------------------------------------------------
+// On-device assembly of G (Eq. 5, Eq. 7): the factored description
+// multiplied out into the canonical CSR arrays the general path takes.  One warp per station pair: the pair's
+// nper rows are cnt * klen elements each and contiguous, so the stores are coalesced; W is read through L1.
+// value = fl(W[q, k] * g_p[t]) (one rounding), column = k * nz + j0_p + t.  HBM-bound: 12 bytes written per nonzero.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, int nz, int klen, const int64_t* __restrict__ lptr,
+                                                      const int32_t* __restrict__ lnode, const double* __restrict__ lw,
+                                                      const int32_t* __restrict__ kj0, const double* __restrict__ kern, int64_t ms,
+                                                      const int64_t* __restrict__ sptr, const int32_t* __restrict__ sidx,
+                                                      const double* __restrict__ sval, int64_t* __restrict__ rowptr,
+                                                      int32_t* __restrict__ colind, double* __restrict__ vals) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int64_t per_entry = (int64_t)nper * klen;
+  for (int64_t q = warp; q < npairs; q += nwarps) {
+    const int64_t e0 = lptr[q], e1 = lptr[q + 1];
+    const int64_t cnt = e1 - e0, rowlen = cnt * klen, base = e0 * per_entry;
+    if (lane < nper) rowptr[q * nper + lane] = base + (int64_t)lane * rowlen;
+    for (int p = 0; p < nper; ++p) {
+      const int j0 = kj0[p];
+      const double* kp = kern + (size_t)p * klen;
+      const int64_t out = base + (int64_t)p * rowlen;
+      for (int64_t idx = lane; idx < rowlen; idx += 32) {
+        const int64_t i = idx / klen;
+        const int t = (int)(idx - i * klen);
+        colind[out + idx] = lnode[e0 + i] * nz + j0 + t;
+        vals[out + idx] = lw[e0 + i] * kp[t];
+      }
+    }
+  }
+  // the extra block, appended unchanged
+  const int64_t nnz_data = lptr[npairs] * per_entry, mdata = npairs * nper;
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nthreads = (int64_t)gridDim.x * blockDim.x;
+  if (ms > 0) {
+    const int64_t snnz = sptr[ms];
+    for (int64_t r = tid; r <= ms; r += nthreads) rowptr[mdata + r] = nnz_data + sptr[r];
+    for (int64_t e = tid; e < snnz; e += nthreads) { colind[nnz_data + e] = sidx[e]; vals[nnz_data + e] = sval[e]; }
+  } else if (tid == 0) {
+    rowptr[mdata] = nnz_data;
+  }
+}
+
+}  // namespace tomo
+
+namespace tomo {
+
+// ------------------------------------------------------------------------------------------------------------------
+// Fast mode, two-stage contraction (option "two_stage", default on; accumulate = 0 only).  In exact arithmetic
+//     (A_data x)[q, p] = sum_k W[q, k] * S[k, p],        S[k, p] = sum_t g_p[t] * x[k * nz + j0_p + t]
+//     (A_data^T u)[k, j] = sum_p g_p[j - j0_p] * T[k, p],  T[k, p] = sum_q W[q, k] * u[q * nper + p]
+// i.e. the depth contraction is done once per node instead of once per ray entry: klen times fewer products.  The
+// operator applied is W (x) g with UNROUNDED entries; it differs from the stored-CSR operator (entries fl(W g)) by
+// one rounding per entry, which is inside what "fast" claims (plain fp64 sums, any association; DESIGN.md F-fac2).
+// dd mode never takes this path: its bit-for-bit contract is on the rounded entries.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const double* __restrict__ x, double* __restrict__ S, const Scalars* sc,
+                                                    int check_stop) {
+  grid_dependency_wait();
+  if (check_stop && sc->stop) return;
+  const int64_t total = d.nnodes * d.nper;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / d.nper;
+    const int p = (int)(i - k * d.nper);
+    const double* xp = x + k * d.nz + d.kj0[p];
+    const double* kp = d.kern + (size_t)p * d.klen;
+    double s = 0.0;
+    for (int t = 0; t < d.klen; ++t) s = fma(kp[t], xp[t], s);
+    S[i] = s;
+  }
+  grid_launch_dependents();
+}
+
+// Entries [e0, e1) of a CSR / CSC list of W, for lane (g, p) the entries g, g + G, ... in order: use(weight, gather(index)).
+// The entries go by in coalesced batches of SB = 32 / G steps (lane l loads entry l of the batch, one batch ahead; the
+// groups pick theirs up by shuffle), the gathers of U steps are in flight before they are used.  (Issuing the next
+// batch's gathers before the current batch is consumed was measured slower: 9.0 k -> 7.6 k it/s at config 1.)
+template <int U, typename GATHER, typename USE>
+__device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const double* __restrict__ val, int64_t e0, int64_t e1, int G, int g,
+                                          bool active, int lane, GATHER gather, USE use) {
+  const int SB = 32 / G, BE = SB * G;
+  int64_t eb = e0;
+  int ireg = 0;
+  double wreg = 0.0;
+  if (lane < BE && eb + lane < e1) { ireg = idx[eb + lane]; wreg = val[eb + lane]; }
+  while (eb < e1) {
+    const int nb = (int)((e1 - eb < (int64_t)BE) ? (e1 - eb) : (int64_t)BE);
+    const int64_t en = eb + BE;
+    int in = 0;
+    double wn = 0.0;
+    if (lane < BE && en + lane < e1) { in = idx[en + lane]; wn = val[en + lane]; }
+    for (int st = 0; st * G < nb; st += U) {
+      double xs[U], ws[U];
+      bool ok[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int src = (st + u) * G + g;
+        ok[u] = active && src < nb;
+        const int i = __shfl_sync(0xffffffffu, ireg, src & 31);
+        ws[u] = __shfl_sync(0xffffffffu, wreg, src & 31);
+        xs[u] = ok[u] ? gather(i) : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        if (ok[u]) use(ws[u], xs[u]);
+    }
+    ireg = in; wreg = wn; eb = en;
+  }
+}
+
+template <int OP>   // OP_PLAIN, OP_K1
+__global__ void __launch_bounds__(kFacThreads, 1)
+k_fac2_rows(const FacDesc d, const double* __restrict__ S, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
+  __shared__ double2 s_slots[kFacWarps];
+  __shared__ int s_flag;
+  constexpr bool K1 = (OP == OP_K1);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  const int gw = blockIdx.x * nwarp + warp, NW = gridDim.x * nwarp;
+  const int nper = d.nper, G = d.G;
+  const int p = lane % nper, g = lane / nper;
+  const bool active = g < G;
+  const int q0 = d.pw[gw], q1 = d.pw[gw + 1];
+  const int64_t x0 = d.ms * gw / NW, x1 = d.ms * (int64_t)(gw + 1) / NW;
+  grid_dependency_wait();
+  const long long t_start = clock64();
+  double c = 0.0, sy = 1.0;
+  if (K1) {
+    if (sc->stop) return;
+    c = -sc->alpha; sy = sc->rbeta;
+  }
+  Acc<0> nsq;
+  nsq.zero();
+  int q_next = (q0 < q1) ? d.pq[q0] : 0;
+  for (int i = q0; i < q1; ++i) {
+    const int q = q_next;
+    if (i + 1 < q1) q_next = d.pq[i + 1];
+    const int64_t r = (int64_t)q * nper + lane;
+    const double yo = (K1 && lane < nper) ? y[r] * sy : 0.0;
+    Acc<0> a;
+    a.zero();
+    fac2_walk<10>(d.lnode, d.lw, d.lptr[q], d.lptr[q + 1], G, g, active, lane,
+                 [&](int k) { return S[(int64_t)k * nper + p]; }, [&](double w, double sv) { a.mac(w, sv); });
+    for (int gg = 1; gg < G; ++gg) {
+      const Acc<0> o = a.down(gg * nper);
+      if (g == 0) a.merge(o);
+    }
+    if (lane < nper) y[r] = fac_finish<0, K1, K1>(a, c, yo, nsq);
+  }
+  for (int64_t r = x0 + lane; r < x1; r += 32) {
+    Acc<0> a;
+    a.zero();
+    for (int64_t e = d.sptr[r]; e < d.sptr[r + 1]; ++e) a.mac(d.sval[e], x[d.sidx[e]]);
+    const int64_t ro = d.mdata + r;
+    const double yo = K1 ? y[ro] * sy : 0.0;
+    y[ro] = fac_finish<0, K1, K1>(a, c, yo, nsq);
+  }
+  if (lane == 0) d.busy[gw] = clock64() - t_start;
+  if (!K1) return;
+  lanes_reduce<32, 0>(nsq);
+  if (lane == 0) s_slots[warp] = nsq.pack();
+  __syncthreads();
+  grid_launch_dependents();
+  if (threadIdx.x == 0) {
+    Acc<0> tot = fac_acc_of<0>(s_slots[0]);
+    for (int i = 1; i < nwarp; ++i) tot.merge(fac_acc_of<0>(s_slots[i]));
+    __stcg(partials + blockIdx.x, tot.pack());
+  }
+  if (!fac_ticket(sc, &s_flag)) return;
+  const double total = final_sum<0>(partials, (int)gridDim.x, s_slots);
+  if (threadIdx.x == 0) {
+    tail_k1(sc, total);
+    sc->ticket[0] = 0u;
+  }
+}
+
+template <int OP>   // OP_PLAIN, OP_K2, OP_K2_INIT
+__global__ void __launch_bounds__(kFacThreads, 1)
+k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
+  __shared__ double s_T[kFacWarps][64];   // per warp: [0, 32) the lanes' sums, [32, 64) the node's T[p]
+  __shared__ double2 s_slots[kFacWarps];
+  __shared__ int s_kj0[32];
+  __shared__ int s_flag;
+  constexpr bool NORM = (OP != OP_PLAIN), AXPY = (OP == OP_K2), SCALE = (OP != OP_PLAIN);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int gw = blockIdx.x * (blockDim.x >> 5) + warp;
+  const int nper = d.nper, G = d.G, nz = d.nz, klen = d.klen;
+  const int p = lane % nper, g = lane / nper;
+  const bool active = g < G;
+  double* my = s_T[warp];
+  if (threadIdx.x < 32) s_kj0[threadIdx.x] = (threadIdx.x < nper) ? d.kj0[threadIdx.x] : 0;
+  const int s0 = d.wseg[gw], s1 = d.wseg[gw + 1];
+  __syncthreads();
+  grid_dependency_wait();
+  double c = 0.0, sx = 1.0;
+  if (OP != OP_PLAIN) {
+    if (sc->stop) return;
+    if (OP == OP_K2 && sc->beta_zero) {
+      if (blockIdx.x == 0 && threadIdx.x == 0) tail_k2(sc, 0.0);
+      return;
+    }
+    if (OP == OP_K2) c = -sc->beta;
+    sx = sc->rbeta;
+  }
+  const long long t_start = clock64();
+  FacSeg sg_next = {};
+  if (s0 < s1) sg_next = d.seg[s0];
+  for (int s = s0; s < s1; ++s) {
+    const FacSeg sg = sg_next;
+    if (s + 1 < s1) sg_next = d.seg[s + 1];
+    const int node = sg.node;
+    int64_t xc0 = 0, xc1 = 0;
+    if (d.scptr && lane < nz) { const int64_t colp = (int64_t)node * nz + lane; xc0 = d.scptr[colp]; xc1 = d.scptr[colp + 1]; }
+    Acc<0> a;
+    a.zero();
+    fac2_walk<10>(d.cpair, d.cw, sg.e0, sg.e1, G, g, active, lane,
+                 [&](int q) { const double xe = x[(int64_t)q * nper + p]; return SCALE ? xe * sx : xe; },
+                 [&](double w, double us) { a.mac(w, us); });
+    for (int gg = 1; gg < G; ++gg) {     // T[p] of this piece in lanes 0 .. nper-1 (groups in index order)
+      const Acc<0> o = a.down(gg * nper);
+      if (g == 0) a.merge(o);
+    }
+    bool closer = sg.nsegs == 1;
+    double T = a.value();
+    if (!closer) {    // a cut node: publish this piece's T, the last piece to arrive adds them in slot order
+      if (lane < nper) __stcg(d.seg_part + (size_t)sg.slot * d.pstride + lane, make_double2(T, 0.0));
+      __threadfence();
+      __syncwarp();
+      unsigned int old = 0;
+      if (lane == 0) old = atomicAdd(d.node_cnt + node, 1u);
+      old = __shfl_sync(0xffffffffu, old, 0);
+      if (old == (unsigned int)(sg.nsegs - 1)) {
+        __threadfence();
+        closer = true;
+        if (lane == 0) d.node_cnt[node] = 0u;
+        if (lane < nper) {
+          const double2* base = d.seg_part + (size_t)(sg.slot - sg.rank) * d.pstride + lane;
+          T = __ldcg(base).x;
+          for (int r = 1; r < sg.nsegs; ++r) T = T + __ldcg(base + (size_t)r * d.pstride).x;
+        }
+      }
+    }
+    if (closer) {
+      if (lane < nper) my[32 + lane] = T;
+      __syncwarp();
+      Acc<0> nsq;
+      nsq.zero();
+      for (int j = lane; j < nz; j += 32) {
+        const int64_t col = (int64_t)node * nz + j;
+        const double yo = AXPY ? y[col] : 0.0;
+        Acc<0> S;
+        S.zero();
+        for (int pp = 0; pp < nper; ++pp) {     // the depth contraction: periods ascending
+          const int t = j - s_kj0[pp];
+          if (t >= 0 && t < klen) S.mac(d.kern[(size_t)pp * klen + t], my[32 + pp]);
+        }
+        if (d.scptr) {
+          const int64_t c0 = (j == lane) ? xc0 : d.scptr[col], c1 = (j == lane) ? xc1 : d.scptr[col + 1];
+          for (int64_t base = c0; base < c1; base += 8) {
+            int32_t rr[8];
+            double vv[8], xe[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const bool in = base + i < c1;
+              rr[i] = in ? d.srow[base + i] : 0;
+              vv[i] = in ? d.scval[base + i] : 0.0;
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) xe[i] = (base + i < c1) ? x[d.mdata + rr[i]] : 0.0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              if (base + i < c1) S.mac(vv[i], SCALE ? xe[i] * sx : xe[i]);
+          }
+        }
+        y[col] = fac_finish<0, AXPY, NORM>(S, c, yo, nsq);
+      }
+      if (NORM) {
+        lanes_reduce<32, 0>(nsq);
+        if (lane == 0) __stcg(d.node_nsq + node, nsq.pack());
+      }
+    }
+    __syncwarp();
+  }
+  if (lane == 0) d.busy[gw] = clock64() - t_start;
+  if (!NORM) return;
+  __threadfence();
+  __syncthreads();
+  grid_launch_dependents();
+  if (!fac_ticket(sc, &s_flag)) return;
+  const double total = final_sum<0>(d.node_nsq, (int)d.nnodes, s_slots);
+  if (threadIdx.x == 0) {
+    if (OP == OP_K2) tail_k2(sc, total);
+    if (OP == OP_K2_INIT) tail_init_v(sc, total);
+    sc->ticket[0] = 0u;
+  }
 }
 
 }  // namespace tomo

@@ -71,14 +71,15 @@ struct Dir {
 // the factored sensitivity block (factored.cuh; tomo_lsqr_create_factored): what the handle owns of it
 struct FacState {
   FacDesc d = {};                 // the kernel argument (borrowed W / A_extra CSR arrays, owned rest)
-  FacDesc dm[2];                  // ... per accumulation mode: the A^T x work split differs (wseg, seg)
+  FacDesc dm[3];                  // ... per mode (0 fast, 1 dd, 2 fast two-stage): the A^T x work split differs (wseg, seg)
+  double* S2 = nullptr;           // two-stage fast mode: S[k, p], the depth contraction of x per node and period
   int64_t E = 0, snnz = 0;        // lateral entries, entries of the extra rows
   int klp = 0; bool guard = false;  // kernel shape: window length as a template constant (8, 12, 16) or the general one (32, guarded)
   int nsegs = 0, nslots = 0;
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
-  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[2] = {nullptr, nullptr}; FacSeg* seg[2] = {nullptr, nullptr};
+  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[3] = {nullptr, nullptr, nullptr}; FacSeg* seg[3] = {nullptr, nullptr, nullptr};
   double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
 };
 
@@ -112,7 +113,7 @@ struct tomo_lsqr_s {
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t gexec = nullptr; int graph_k = 0, graph_mode = -1, graph_G = 0;
   // options
-  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 320, pdl = 1, compress = 0;
+  int check_every = 10, accumulate = 1, use_graph = 1, profile = 0, row_cost = 320, pdl = 1, compress = 0, two_stage = 1;
   // info
   int sms = 0; double create_ms = 0, transpose_ms = 0, transpose_kernels_ms = 0, update_ms = 0, scratch_bytes = 0;
   double2* sh_send = nullptr; double2* sh_recv = nullptr; int64_t sh_send_cap = 0, sh_recv_cap = 0;  // exchange buffers of the sharded solve
@@ -246,9 +247,35 @@ cudaError_t launch_fac_mode(const tomo_lsqr_s* h, bool cols, const double* x, do
     default: return launch_fac_one<MODE, OP, 32, true>(h, cols, x, y, st);
   }
 }
+// fast mode, two-stage contraction (k_fac2_*): the depth contraction once per node, then W
+template <int OP>
+cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double* y, cudaStream_t st) {
+  const FacState* f = h->fac;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.stream = st; cfg.attrs = at; cfg.numAttrs = (h->pdl && OP != OP_PLAIN) ? 1 : 0;
+  cfg.blockDim = dim3(kFacThreads); cfg.gridDim = dim3((unsigned)h->sms);
+  if (cols) {
+    if constexpr (OP == OP_PLAIN || OP == OP_K2 || OP == OP_K2_INIT)
+      return cudaLaunchKernelEx(&cfg, k_fac2_cols<OP>, f->dm[2], x, y, h->sc, h->part_spmv);
+  } else {
+    if constexpr (OP == OP_PLAIN || OP == OP_K1) {
+      cudaLaunchConfig_t c1 = cfg;
+      c1.blockDim = dim3(256);
+      c1.gridDim = dim3((unsigned)std::max<int64_t>(1, std::min<int64_t>((f->d.nnodes * f->d.nper + 255) / 256, (int64_t)h->sms * 8)));
+      cudaError_t e = cudaLaunchKernelEx(&c1, k_fac2_stage, f->dm[2], x, f->S2, (const Scalars*)h->sc, OP == OP_K1 ? 1 : 0);
+      if (e != cudaSuccess) return e;
+      return cudaLaunchKernelEx(&cfg, k_fac2_rows<OP>, f->dm[2], (const double*)f->S2, x, y, h->sc, h->part_spmv);
+    }
+  }
+  return cudaErrorInvalidValue;
+}
 template <int OP>
 void launch_fac(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
   if (h->accumulate) launch_fac_mode<1, OP>(h, transpose, x, y, st);
+  else if (h->two_stage) launch_fac2<OP>(h, transpose, x, y, st);
   else launch_fac_mode<0, OP>(h, transpose, x, y, st);
 }
 // the > 48 KB dynamic shared memory opt-in of the k_fac_cols instantiations on the current device
@@ -471,7 +498,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
     cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
-    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); for (int i = 0; i < 2; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->S2); for (int i = 0; i < 3; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
     cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
   }
@@ -703,10 +730,10 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     std::vector<int64_t> cptr((size_t)nnodes + 1);
     if ((e = cudaMemcpyAsync(cptr.data(), f->cptr, sizeof(int64_t) * (nnodes + 1), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the node pointers"); break; }
-    std::vector<FacSeg> segs_m[2];
-    std::vector<int32_t> wseg_m[2];
+    std::vector<FacSeg> segs_m[3];
+    std::vector<int32_t> wseg_m[3];
     int nslots_max = 0;
-    for (int mode = 0; mode < 2; ++mode) {
+    for (int mode = 0; mode < 3; ++mode) {
       std::vector<FacSeg>& segs = segs_m[mode];
       std::vector<int32_t>& wseg = wseg_m[mode];
       std::vector<int32_t> owner;
@@ -716,7 +743,8 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       // node whose entries straddle a boundary is cut there (pieces of at least kMinPiece entries).
       // measured on B200 (per-warp busy cycles): closing a node is a chain of dependent loads worth ~5 k cycles,
       // i.e. the time of ~26 entries in dd mode and ~55 in fast mode, hence one split per mode
-      const double kClose = mode ? 26.0 : 55.0, kCloseEmpty = mode ? 14.0 : 28.0;
+      // (two-stage fast mode: an entry is one FMA, the closing is the same chain: ~250 entries)
+      const double kClose = mode == 1 ? 26.0 : mode == 0 ? 55.0 : 250.0, kCloseEmpty = mode == 1 ? 14.0 : mode == 0 ? 28.0 : 125.0;
       const int64_t kMinPiece = 8;
       int64_t empty = 0;
       for (int64_t k = 0; k < nnodes; ++k) empty += cptr[k] == cptr[k + 1];
@@ -761,7 +789,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     }
     ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->pq, sizeof(int32_t) * npairs);
     if ((e = cudaMemcpyAsync(f->pq, pq.data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the pair lists"); break; }
-    for (int mode = 0; mode < 2 && rc == TOMO_OK; ++mode) {
+    for (int mode = 0; mode < 3 && rc == TOMO_OK; ++mode) {
       if ((e = cudaMalloc(&f->wseg[mode], sizeof(int32_t) * (NW + 1))) != cudaSuccess ||
           (e = cudaMalloc(&f->seg[mode], sizeof(FacSeg) * std::max<size_t>(segs_m[mode].size(), 1))) != cudaSuccess ||
           (e = cudaMemcpyAsync(f->wseg[mode], wseg_m[mode].data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
@@ -769,7 +797,8 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
         rc = cuda_fail(e, "upload of the A^T x work split");
     }
     if (rc != TOMO_OK) break;
-    ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(nslots_max, 1) * nz);
+    ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(nslots_max, 1) * std::max<int>(nz, nper));
+    ALLOC(f->S2, sizeof(double) * nnodes * nper);
     ALLOC(f->node_cnt, sizeof(unsigned int) * nnodes); ALLOC(f->node_nsq, sizeof(double2) * nnodes);
     ALLOC(f->busy, sizeof(long long) * NW);
     if ((e = cudaMemsetAsync(f->busy, 0, sizeof(long long) * NW, st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
@@ -802,7 +831,8 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     d.scptr = f->scptr; d.srow = f->srow; d.scval = f->scval;
     d.pw = f->pw; d.pq = f->pq; d.wseg = f->wseg[1]; d.seg = f->seg[1];
     d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq; d.busy = f->busy;
-    for (int mode = 0; mode < 2; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
+    d.pstride = std::max<int>(nz, nper);
+    for (int mode = 0; mode < 3; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
     cudaEventRecord(e1, st);
     if ((e = cudaEventSynchronize(e1)) != cudaSuccess) { rc = cuda_fail(e, "create_factored"); break; }
     float msf = 0;
@@ -813,6 +843,43 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
   if (e1) cudaEventDestroy(e1);
   if (rc != TOMO_OK) { free_handle(h); return rc; }
   *out = h;
+  return TOMO_OK;
+}
+
+// NEXT-4: on-device assembly of G from its factored description (k_fac_assemble)
+extern "C" tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz, const int64_t* d_lptr,
+                                                const int32_t* d_lnode, const double* d_lw, int32_t klen, const int32_t* d_kj0,
+                                                const double* d_kern, int64_t ms, int64_t snnz, const int64_t* d_sptr,
+                                                const int32_t* d_sidx, const double* d_svals, int64_t nnz, int64_t* d_rowptr,
+                                                int32_t* d_colind, double* d_vals, void* cuda_stream) {
+  if (npairs < 1 || nnodes < 1 || nz < 1 || nper < 1 || klen < 1 || ms < 0 || snnz < 0 || nnz < 0) return TOMO_ERR_INVALID_ARG;
+  if (nper > 32 || klen > 32 || klen > nz) return TOMO_ERR_RANGE;
+  if ((double)npairs * nper + (double)ms >= (double)INT32_MAX || (double)nnodes * nz >= (double)INT32_MAX) return TOMO_ERR_RANGE;
+  if (!d_lptr || !d_kj0 || !d_kern || !d_rowptr || (ms > 0 && !d_sptr) || (snnz > 0 && (!d_sidx || !d_svals || ms == 0)) ||
+      (nnz > 0 && (!d_colind || !d_vals)))
+    return TOMO_ERR_INVALID_ARG;
+  int dev = 0, major = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) return TOMO_ERR_UNSUPPORTED_ARCH;
+  if (!is_device_ptr(d_lptr) || !is_device_ptr(d_kj0) || !is_device_ptr(d_kern) || !is_device_ptr(d_rowptr) ||
+      (ms > 0 && !is_device_ptr(d_sptr)) || (snnz > 0 && (!is_device_ptr(d_sidx) || !is_device_ptr(d_svals))) ||
+      (nnz > 0 && (!is_device_ptr(d_colind) || !is_device_ptr(d_vals))))
+    return TOMO_ERR_NOT_DEVICE_PTR;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // the caller's nnz must be the size of the assembled matrix: entries of W x nper x klen + the extra block
+  int64_t E = 0, sn = 0;
+  CK(cudaMemcpyAsync(&E, d_lptr + npairs, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  if (ms > 0) CK(cudaMemcpyAsync(&sn, d_sptr + ms, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (E < 0 || sn != snnz || E * (int64_t)nper * klen + snnz != nnz) return TOMO_ERR_INVALID_ARG;
+  if (E > 0 && (!d_lnode || !d_lw)) return TOMO_ERR_INVALID_ARG;
+  if (E > 0 && (!is_device_ptr(d_lnode) || !is_device_ptr(d_lw))) return TOMO_ERR_NOT_DEVICE_PTR;
+  k_fac_assemble<<<sms * 8, 256, 0, st>>>(npairs, nper, nz, klen, d_lptr, d_lnode, d_lw, d_kj0, d_kern, ms, d_sptr, d_sidx, d_svals,
+                                         d_rowptr, d_colind, d_vals);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(st));
   return TOMO_OK;
 }
 
@@ -831,7 +898,7 @@ void enqueue_iteration(const tomo_lsqr_s* h, cudaStream_t st) {
 }
 
 tomo_status_t ensure_graph(tomo_lsqr_s* h) {
-  const int gkey = h->accumulate + 2 * h->solver;
+  const int gkey = h->accumulate + 2 * h->solver + 4 * h->two_stage;
   if (h->gexec && h->graph_k == h->check_every && h->graph_mode == gkey && h->graph_G == h->SG) return TOMO_OK;
   if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
   cudaGraph_t g = nullptr;
@@ -915,7 +982,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
       }
       CK(cudaGetLastError());
     }
-    h->kernels_enqueued += 3.0 * k;
+    h->kernels_enqueued += (h->fac && !h->accumulate && h->two_stage ? 4.0 : 3.0) * k;   // the two-stage A x is two launches
     // host poll: {itn, istop, stop}.  The next replay is enqueued before this one is inspected, so the
     // device never idles on the host; kernels after a stop return at once and leave x frozen.
     CK(cudaMemcpyAsync(&h->h_poll[slot], &h->sc->itn, sizeof(PollWord), cudaMemcpyDeviceToHost, st));
@@ -1471,6 +1538,7 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
+  else if (k == "two_stage") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->two_stage = (int)value; }
   else if (k == "multi_shared") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->multi_shared = (int)value; }
   else if (k == "compress") {
     if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG;

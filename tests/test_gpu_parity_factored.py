@@ -71,8 +71,8 @@ def test_factored_spmv_and_solve_random_shapes(tl, shape):
     assert (S.m, S.n) == (m, n) and S.info("factored") == 1.0 and S.info("lateral_entries") == len(f["lnode"])
     rng = np.random.default_rng(shape[0])
     x, u = rng.standard_normal(n), rng.standard_normal(m)
-    for acc, mode, in ((1, oracle.DD), (0, oracle.PLAIN)):
-        S.set(accumulate=acc)
+    for acc, mode, ts in ((1, oracle.DD, 1), (0, oracle.PLAIN, 1), (0, oracle.PLAIN, 0)):   # ts: fast mode's two-stage contraction / per-entry products
+        S.set(accumulate=acc, two_stage=ts)
         y = S.spmv(dev(x)).cpu().numpy()
         yt = S.spmv(dev(u), transpose=True).cpu().numpy()
         oy, oyt = oracle.spmv(m, n, rp, ci, va, x, mode), oracle.spmv_t(m, n, rp, ci, va, u, mode)
@@ -119,6 +119,12 @@ def test_factored_cfg0_both_modes(tl, cfg0):
     xg, res = S.solve(dev(b), damp=s.damp, atol=1e-6, btol=1e-6, max_iters=300)
     o = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, atol=1e-6, btol=1e-6, max_iters=300, mode=oracle.DD)
     assert (res.itn, res.istop) == (o.itn, o.istop) and np.array_equal(xg.cpu().numpy(), o.x)
+    # fast mode without the two-stage contraction (per-entry products of the rounded values): same bar
+    S.set(accumulate=0, two_stage=0)
+    xg, res = S.solve(dev(b), damp=s.damp, max_iters=50)
+    o = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=50, mode=oracle.PLAIN)
+    assert res.itn == 50 and rel(xg.cpu().numpy(), o.x) <= TOL_X50
+    S.set(two_stage=1)
     # determinism and independence of the launch mode (graph / check_every / pdl), both accumulation modes
     for acc in (1, 0):
         S.set(accumulate=acc, graph=1, check_every=10, pdl=1)
@@ -287,3 +293,57 @@ def test_factored_cfg2_full_size(tl):
         pytest.skip("config-2 x_k parity of the factored operator not run: " + o["skipped"])
     for k, want in ((1, o["snapshots"][1]), (2, o["snapshots"][2]), (5, o["x"])):
         assert rel(xk[k], want) <= TOL_X50 and np.array_equal(xk[k], want), k
+
+
+def assemble(tl, f):
+    """tomo_lsqr_assemble_csr on the device -> (rowptr, colind, vals) device tensors."""
+    ms = 0 if f["sptr"] is None else len(f["sptr"]) - 1
+    snnz = 0 if f["sidx"] is None else len(f["sidx"])
+    m = f["npairs"] * f["nper"] + ms
+    nnz = len(f["lnode"]) * f["nper"] * f["klen"] + snnz
+    keep = [dev(f[k]) for k in ("lptr", "lnode", "lw")] + [dev(f["kj0"].astype(np.int32)), dev(f["kern"])] + \
+           [dev(f[k]) for k in ("sptr", "sidx", "svals")]
+    rp = torch.full((m + 1,), -1, dtype=torch.int64, device="cuda")
+    ci = torch.full((max(nnz, 1),), -1, dtype=torch.int32, device="cuda")
+    va = torch.full((max(nnz, 1),), float("nan"), dtype=torch.float64, device="cuda")
+    tl.tomo_lsqr_assemble_csr(f["npairs"], f["nper"], f["nnodes"], f["nz"], keep[0], keep[1], keep[2], f["klen"], keep[3], keep[4],
+                              ms, snnz, keep[5], keep[6], keep[7], nnz, rp, ci, va)
+    return m, nnz, rp, ci[:nnz], va[:nnz]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_assemble_csr_random_shapes(tl, shape):
+    """NEXT-4, on-device assembly of G: bit-exact (indices and one-rounding values) against the oracle's expansion."""
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=2000 + npairs, ms=ms)
+    orp, oci, ova = expand(f)
+    m, nnz, rp, ci, va = assemble(tl, f)
+    assert np.array_equal(rp.cpu().numpy(), orp) and np.array_equal(ci.cpu().numpy(), oci) and np.array_equal(va.cpu().numpy(), ova)
+
+
+def test_assemble_csr_configs_and_roundtrip(tl, cfg0):
+    import paper_2604_11920_b200 as T
+    # config 0: equals the generator's host assembly; the assembled matrix is accepted by tomo_lsqr_create and solves to
+    # the bits of the factored handle
+    s = cfg0["sys"]
+    f = s.factored()
+    m, nnz, rp, ci, va = assemble(tl, f)
+    assert np.array_equal(rp.cpu().numpy(), cfg0["rp"]) and np.array_equal(ci.cpu().numpy(), cfg0["ci"]) and np.array_equal(va.cpu().numpy(), cfg0["va"])
+    C = tl.TomoLsqr(m, cfg0["n"], rp, ci, va)
+    F = make(tl, f)
+    b = dev(cfg0["b"])
+    assert torch.equal(C.solve(b, damp=s.damp, max_iters=50)[0], F.solve(b, damp=s.damp, max_iters=50)[0])
+    C.close(); F.close()
+    # config 1 at full size (194 M nonzeros, 2.3 GB written): equals the generator's CSR
+    s1 = tomogen.System(1)
+    f1 = s1.factored()
+    m, nnz, rp, ci, va = assemble(tl, f1)
+    orp, oci, ova = s1.csr()
+    assert nnz == s1.dims.nnz and np.array_equal(rp.cpu().numpy(), orp)
+    assert torch.equal(ci, dev(oci)) and torch.equal(va, dev(ova))
+    # a wrong nnz is refused before anything is written
+    with pytest.raises(T.TomoError) as ei:
+        T.tomo_lsqr_assemble_csr(f["npairs"], f["nper"], f["nnodes"], f["nz"], dev(f["lptr"]), dev(f["lnode"]), dev(f["lw"]), f["klen"],
+                                 dev(f["kj0"]), dev(f["kern"]), len(f["sptr"]) - 1, len(f["sidx"]), dev(f["sptr"]), dev(f["sidx"]),
+                                 dev(f["svals"]), 7, rp, ci, va)
+    assert ei.value.status == T.TOMO_ERR_INVALID_ARG
