@@ -93,9 +93,10 @@ tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t n
  * A lateral entry (12 bytes) stands for nper * klen nonzeros of the CSR form, so the products are bound by fp64
  * arithmetic instead of HBM (get_info "operator_bytes").  Every product uses the ROUNDED value fl(W g), the number the
  * CSR form stores: with "accumulate" = 1 all results (tomo_lsqr_spmv, the solves) are bit for bit those of a
- * tomo_lsqr_create handle on the expanded matrix; with "accumulate" = 0 they agree to rounding (other summation order).
+ * tomo_lsqr_create handle on the expanded matrix; with "accumulate" = 0 they agree to rounding (other summation order and,
+ * with option "two_stage" = 1, the unrounded entries W g).
  * Supported on such a handle: tomo_lsqr_solve / tomo_lsmr_solve, *_solve_host, *_solve_multi (the sides run one after
- * the other), tomo_lsqr_spmv, the options "check_every", "accumulate", "graph", "profile", "pdl", and get_info.
+ * the other), tomo_lsqr_spmv, the options "check_every", "accumulate", "graph", "profile", "pdl", "two_stage", and get_info.
  * Not supported (INVALID_ARG): tomo_lsqr_update_values (nothing is stored per nonzero: create again, it costs
  * milliseconds), tomo_lsqr_get_csc, "compress" = 1, tomo_lsqr_solve_sharded.
  * Errors: INVALID_ARG, RANGE, NOT_DEVICE_PTR, BAD_CSR (W, A_extra or the kernel table malformed / non-finite),
@@ -211,6 +212,12 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *                          ordering of PAPER.md Eq. 7 P:79 makes every lateral node of a ray a run of consecutive
  *                          columns, Eq. 5) and streams those instead of the int32 arrays.  Same elements,
  *                          same order: results are bitwise those of "compress" = 0.  Default 0.
+ *   "two_stage"   0 | 1    factored handles, "accumulate" = 0 only (default 1): apply A_data as W after the depth contraction
+ *                          S[k, p] = sum_t g_p[t] x[k nz + j0_p + t] (and A_data^T as the contraction of T[k, p] = sum_q W[q, k]
+ *                          u[q nper + p]): klen times fewer products.  The operator applied has the UNROUNDED entries W g
+ *                          (one rounding per entry away from the CSR form's fl(W g)); results stay within the fast-mode
+ *                          bar (SpMV 1e-12, x_k as any other summation order).  0: per-entry products of the rounded values.
+ *                          Never used with "accumulate" = 1, whose results are bit for bit those of the CSR form.
  *   "pdl"         0 | 1    chain the kernels of an iteration with programmatic dependent launch (default 1): the
  *                          prologue of a kernel (barrier set-up, split points, first bulk copies) overlaps the
  *                          tail of the previous one; never changes results
