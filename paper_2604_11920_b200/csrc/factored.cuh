@@ -427,6 +427,7 @@ __global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, 
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
   const int64_t per_entry = (int64_t)nper * klen;
+  const int di = 32 / klen, dt = 32 - di * klen;
   for (int64_t q = warp; q < npairs; q += nwarps) {
     const int64_t e0 = lptr[q], e1 = lptr[q + 1];
     const int64_t cnt = e1 - e0, rowlen = cnt * klen, base = e0 * per_entry;
@@ -435,11 +436,14 @@ __global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, 
       const int j0 = kj0[p];
       const double* kp = kern + (size_t)p * klen;
       const int64_t out = base + (int64_t)p * rowlen;
+      // element idx = i * klen + t of the row; the lane steps by 32 elements: (i, t) advance without a division
+      int64_t i = lane / klen;
+      int t = lane - (int)i * klen;
       for (int64_t idx = lane; idx < rowlen; idx += 32) {
-        const int64_t i = idx / klen;
-        const int t = (int)(idx - i * klen);
         colind[out + idx] = lnode[e0 + i] * nz + j0 + t;
         vals[out + idx] = lw[e0 + i] * kp[t];
+        i += di; t += dt;
+        if (t >= klen) { t -= klen; ++i; }
       }
     }
   }
