@@ -41,6 +41,12 @@ def _load():
         lib.oracle_spmv.restype = None
         lib.oracle_spmv_t.argtypes = [i64, i64, vp, vp, vp, vp, vp, ci]
         lib.oracle_spmv_t.restype = None
+        lib.oracle_spmv_x.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp, ci]
+        lib.oracle_spmv_x.restype = None
+        lib.oracle_spmv_t_x.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp, ci]
+        lib.oracle_spmv_t_x.restype = None
+        lib.oracle_lsqr_solve_x.argtypes = [i64, i64, vp, vp, vp, vp, vp, f64, f64, f64, i32, ci, vp, vp, vp, vp, i32, vp, vp]
+        lib.oracle_lsqr_solve_x.restype = None
         lib.oracle_csr_to_csc.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp]
         lib.oracle_csr_to_csc.restype = None
         lib.oracle_lsqr_new.argtypes = [i64, i64, vp, vp, vp, vp, f64, f64, f64, i32, ci]
@@ -74,18 +80,27 @@ def _csr(rowptr, colind, vals):
     return rp, ci, va
 
 
-def spmv(m, n, rowptr, colind, vals, x, mode=PLAIN):
+def spmv(m, n, rowptr, colind, vals, x, mode=PLAIN, vals_lo=None):
+    """vals_lo: optional second word of every entry (entry = vals + vals_lo, dd mode; oracle/factored.py expand_exact)."""
     rp, ci, va = _csr(rowptr, colind, vals)
     x = np.ascontiguousarray(x, dtype=np.float64)
     y = np.empty(m, dtype=np.float64)
+    if vals_lo is not None:
+        lo = np.ascontiguousarray(vals_lo, dtype=np.float64)
+        _load().oracle_spmv_x(m, n, _p(rp), _p(ci), _p(va), _p(lo), _p(x), _p(y), mode)
+        return y
     _load().oracle_spmv(m, n, _p(rp), _p(ci), _p(va), _p(x), _p(y), mode)
     return y
 
 
-def spmv_t(m, n, rowptr, colind, vals, u, mode=PLAIN):
+def spmv_t(m, n, rowptr, colind, vals, u, mode=PLAIN, vals_lo=None):
     rp, ci, va = _csr(rowptr, colind, vals)
     u = np.ascontiguousarray(u, dtype=np.float64)
     v = np.empty(n, dtype=np.float64)
+    if vals_lo is not None:
+        lo = np.ascontiguousarray(vals_lo, dtype=np.float64)
+        _load().oracle_spmv_t_x(m, n, _p(rp), _p(ci), _p(va), _p(lo), _p(u), _p(v), mode)
+        return v
     _load().oracle_spmv_t(m, n, _p(rp), _p(ci), _p(va), _p(u), _p(v), mode)
     return v
 
@@ -115,9 +130,11 @@ class Result:
     snapshots: dict
 
 
-def lsqr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, mode=PLAIN, snapshots=()):
-    """Run the oracle LSQR.  ``snapshots``: iteration numbers whose iterate x_k is also returned."""
+def lsqr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, mode=PLAIN, snapshots=(), vals_lo=None):
+    """Run the oracle LSQR.  ``snapshots``: iteration numbers whose iterate x_k is also returned.
+    ``vals_lo``: optional second word of every entry (entry = vals + vals_lo; used in dd mode)."""
     rp, ci, va = _csr(rowptr, colind, vals)
+    lo = None if vals_lo is None else np.ascontiguousarray(vals_lo, dtype=np.float64)
     b = np.ascontiguousarray(b, dtype=np.float64)
     assert len(b) == m and len(rp) == m + 1
     x = np.zeros(n, dtype=np.float64)
@@ -126,9 +143,9 @@ def lsqr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=
     arh = np.full(max(max_iters, 1), np.nan)
     snaps = np.ascontiguousarray(sorted(int(k) for k in snapshots), dtype=np.int32)
     sx = np.full((len(snaps), n), np.nan)
-    _load().oracle_lsqr_solve(m, n, _p(rp), _p(ci), _p(va), _p(b), damp, atol, btol, int(max_iters), mode,
-                              _p(x), _p(res), _p(r2h), _p(arh), len(snaps), _p(snaps) if len(snaps) else None,
-                              _p(sx) if len(snaps) else None)
+    _load().oracle_lsqr_solve_x(m, n, _p(rp), _p(ci), _p(va), _p(lo), _p(b), damp, atol, btol, int(max_iters), mode,
+                                _p(x), _p(res), _p(r2h), _p(arh), len(snaps), _p(snaps) if len(snaps) else None,
+                                _p(sx) if len(snaps) else None)
     itn = int(res[0])
     return Result(x, itn, int(res[1]), res[2], res[3], res[4], res[5], res[6], res[7], r2h[:itn].copy(), arh[:itn].copy(),
                   {int(k): sx[i] for i, k in enumerate(snaps)})

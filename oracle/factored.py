@@ -55,3 +55,36 @@ def expand(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None, sidx
         colind = np.concatenate([colind, np.asarray(sidx, dtype=np.int32)])
         vals = np.concatenate([vals, np.asarray(svals, dtype=np.float64)])
     return rowptr, colind, vals
+
+
+def two_prod(a, b):
+    """(p, e) with p = fl(a * b) and p + e = a * b exactly (Dekker's product through Veltkamp splitting: no FMA needed,
+    exact in fp64 barring over/underflow; elementwise on numpy arrays)."""
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    p = a * b
+    c = 134217729.0  # 2^27 + 1
+    ah = c * a; ah = ah - (ah - a); al = a - ah
+    bh = c * b; bh = bh - (bh - b); bl = b - bh
+    e = ((ah * bh - p) + ah * bl + al * bh) + al * bl
+    return p, e
+
+
+def expand_exact(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None, sidx=None, svals=None):
+    """The factored operator with EXACT entries W[q, k] * g_p[t] (reading F-fac3) as two-word CSR values:
+    (rowptr, colind, vals, vals_lo) with vals = fl(W g) (what `expand` returns) and vals + vals_lo = W g exactly; the
+    extra block's entries are one word (vals_lo = 0).  oracle.spmv / spmv_t / lsqr(..., mode=DD, vals_lo=...) then sum the
+    exact products of both words and round once: the definition  y_i = RN( sum_j (W g)_ij x_j )  written out."""
+    rowptr, colind, vals = expand(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr, sidx, svals)
+    lw = np.asarray(lw, dtype=np.float64)
+    kern = np.asarray(kern, dtype=np.float64).reshape(nper, -1)
+    lptr = np.asarray(lptr, dtype=np.int64)
+    lo = np.zeros_like(vals)
+    for q in range(npairs):
+        w = lw[lptr[q]:lptr[q + 1]]
+        for p in range(nper):
+            r = q * nper + p
+            pr, er = two_prod(w[:, None], kern[p][None, :])
+            assert np.array_equal(pr.reshape(-1), vals[rowptr[r]:rowptr[r + 1]])
+            lo[rowptr[r]:rowptr[r + 1]] = er.reshape(-1)
+    return rowptr, colind, vals, lo

@@ -61,6 +61,10 @@ struct Csr {
   const int64_t* rowptr;
   const int32_t* colind;
   const double* vals;
+  // optional second word of every entry: the entry is the unevaluated sum vals[e] + vals_lo[e] (the factored
+  // operator with exact entries W*g, reading F-fac3: vals = fl(W g), vals_lo = W g - fl(W g) exactly).
+  // Used in dd mode only (the entry's two words are two exact products); NULL: the entry is vals[e].
+  const double* vals_lo = nullptr;
 };
 
 // y_i = sum_j a_ij x_j + c * y_i   (c = 0: plain product; c = -alpha: the LSQR u-update)
@@ -73,7 +77,10 @@ void spmv(const Csr& A, const double* x, double c, double* y, int mode) {
     } else {
       dd acc{0.0, 0.0};
       if (c != 0.0) dd_fma(acc, c, y[i]);
-      for (int64_t e = A.rowptr[i]; e < A.rowptr[i + 1]; ++e) dd_fma(acc, A.vals[e], x[A.colind[e]]);
+      for (int64_t e = A.rowptr[i]; e < A.rowptr[i + 1]; ++e) {
+        dd_fma(acc, A.vals[e], x[A.colind[e]]);
+        if (A.vals_lo) dd_fma(acc, A.vals_lo[e], x[A.colind[e]]);
+      }
       y[i] = dd_round(acc);
     }
   }
@@ -92,7 +99,10 @@ void spmv_t(const Csr& A, const double* u, double c, double* v, int mode, std::v
     if (c != 0.0) for (int64_t j = 0; j < A.n; ++j) dd_fma(work[j], c, v[j]);
     for (int64_t i = 0; i < A.m; ++i) {
       double ui = u[i];
-      for (int64_t e = A.rowptr[i]; e < A.rowptr[i + 1]; ++e) dd_fma(work[A.colind[e]], A.vals[e], ui);
+      for (int64_t e = A.rowptr[i]; e < A.rowptr[i + 1]; ++e) {
+        dd_fma(work[A.colind[e]], A.vals[e], ui);
+        if (A.vals_lo) dd_fma(work[A.colind[e]], A.vals_lo[e], ui);
+      }
     }
     for (int64_t j = 0; j < A.n; ++j) v[j] = dd_round(work[j]);
   }
@@ -374,6 +384,18 @@ void oracle_spmv(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* col
   Csr A{m, n, rowptr, colind, vals};
   spmv(A, x, 0.0, y, mode);
 }
+// the same with two-word entries vals + vals_lo (dd mode)
+void oracle_spmv_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                   const double* x, double* y, int mode) {
+  Csr A{m, n, rowptr, colind, vals, vals_lo};
+  spmv(A, x, 0.0, y, mode);
+}
+void oracle_spmv_t_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                     const double* u, double* v, int mode) {
+  Csr A{m, n, rowptr, colind, vals, vals_lo};
+  std::vector<dd> work;
+  spmv_t(A, u, 0.0, v, mode, work);
+}
 
 // v = A^T u  (scatter over rows)
 void oracle_spmv_t(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
@@ -431,11 +453,26 @@ void oracle_lsqr_get_scalars(void* h, double* out) {
 // Whole solve.  res[0..7] = itn, istop, r1norm, r2norm, arnorm, anorm, acond, xnorm.
 // r2hist / arhist: [max_iters] or NULL.  snap_iters[nsnap] ascending iteration numbers whose x is
 // copied to snap_x[nsnap][n] (NULL for none).
+void oracle_lsqr_solve_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                         const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
+                         double* x, double* res, double* r2hist, double* arhist,
+                         int32_t nsnap, const int32_t* snap_iters, double* snap_x);
 void oracle_lsqr_solve(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
                        const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
                        double* x, double* res, double* r2hist, double* arhist,
                        int32_t nsnap, const int32_t* snap_iters, double* snap_x) {
-  Lsqr* s = (Lsqr*)oracle_lsqr_new(m, n, rowptr, colind, vals, b, damp, atol, btol, max_iters, mode);
+  oracle_lsqr_solve_x(m, n, rowptr, colind, vals, nullptr, b, damp, atol, btol, max_iters, mode, x, res, r2hist, arhist, nsnap, snap_iters,
+                      snap_x);
+}
+// the same on two-word entries vals + vals_lo (NULL: one-word entries)
+void oracle_lsqr_solve_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                         const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
+                         double* x, double* res, double* r2hist, double* arhist,
+                         int32_t nsnap, const int32_t* snap_iters, double* snap_x) {
+  Lsqr* s = new Lsqr();
+  s->A = Csr{m, n, rowptr, colind, vals, vals_lo};
+  s->mode = mode; s->damp = damp; s->atol = atol; s->btol = btol; s->max_iters = max_iters;
+  s->init(b);
   int32_t sn = 0;
   while (!s->done) {
     s->step();

@@ -90,3 +90,76 @@ def test_row_sums_are_ray_lengths():
     sums = np.add.reduceat(va, rp[:d.m_data])
     assert np.allclose(sums, np.repeat(L, d.nper), rtol=1e-13, atol=0)
     assert np.abs(np.add.reduceat(va[rp[d.m_data]:], rp[d.m_data:-1] - rp[d.m_data])).max() < 1e-12   # smoothing rows sum to 0
+
+
+# ---- exact entries W*g as two-word values (reading F-fac3) ---------------------------------------------
+def test_two_prod_is_exact():
+    from fractions import Fraction
+    rng = np.random.default_rng(3)
+    a = rng.standard_normal(500) * 10.0 ** rng.integers(-8, 8, size=500)
+    b = rng.standard_normal(500) * 10.0 ** rng.integers(-8, 8, size=500)
+    p, e = factored.two_prod(a, b)
+    assert np.array_equal(p, a * b)
+    for i in range(500):
+        assert Fraction(float(p[i])) + Fraction(float(e[i])) == Fraction(float(a[i])) * Fraction(float(b[i]))
+
+
+@pytest.mark.parametrize("shape", [(6, 3, 7, 6, 4, None), (5, 10, 6, 20, 12, 9)])
+def test_exact_entries_dd_products_are_the_rounded_exact_sums(shape):
+    """oracle.spmv / spmv_t in dd mode on the two-word entries = the exact rational sum over the UNROUNDED entries W*g,
+    rounded once to nearest; and it differs from the one-word (rounded-entry) result somewhere, so the second word is
+    really used.  Values with a wide exponent spread and cancelling signs."""
+    from fractions import Fraction
+
+    import oracle
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=40 + npairs, ms=ms)
+    rng = np.random.default_rng(9)
+    f["lw"] = f["lw"] * 10.0 ** rng.integers(-3, 4, size=len(f["lw"]))
+    rp, ci, va, lo = factored.expand_exact(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                                           f["sptr"], f["sidx"], f["svals"])
+    m, n = len(rp) - 1, nnodes * nz
+    x = rng.standard_normal(n) * 10.0 ** rng.integers(-2, 3, size=n)
+    u = rng.standard_normal(m) * 10.0 ** rng.integers(-2, 3, size=m)
+    # the exact operator entry by entry from the definition (rational)
+    nperK = f["nper"]
+    exact = {}
+    for q in range(npairs):
+        for e in range(f["lptr"][q], f["lptr"][q + 1]):
+            k, w = int(f["lnode"][e]), Fraction(float(f["lw"][e]))
+            for p in range(nperK):
+                for t in range(klen):
+                    exact[(q * nperK + p, k * nz + int(f["kj0"][p]) + t)] = w * Fraction(float(f["kern"][p][t]))
+    if f["sptr"] is not None:
+        for r in range(len(f["sptr"]) - 1):
+            for e in range(f["sptr"][r], f["sptr"][r + 1]):
+                exact[(npairs * nperK + r, int(f["sidx"][e]))] = Fraction(float(f["svals"][e]))
+    ey = [Fraction(0)] * m
+    ev = [Fraction(0)] * n
+    for (i, j), a in exact.items():
+        ey[i] += a * Fraction(float(x[j]))
+        ev[j] += a * Fraction(float(u[i]))
+    y = oracle.spmv(m, n, rp, ci, va, x, oracle.DD, vals_lo=lo)
+    v = oracle.spmv_t(m, n, rp, ci, va, u, oracle.DD, vals_lo=lo)
+    assert np.array_equal(y, np.array([float(z) for z in ey]))      # float(Fraction) rounds to nearest
+    assert np.array_equal(v, np.array([float(z) for z in ev]))
+    y1 = oracle.spmv(m, n, rp, ci, va, x, oracle.DD)
+    assert not np.array_equal(y, y1) and np.allclose(y, y1, rtol=1e-12, atol=1e-300)
+
+
+def test_exact_entries_lsqr_is_lsqr_on_a_nearby_matrix():
+    """LSQR on the two-word entries: x_k within rounding-level perturbation theory of the one-word run (the matrices differ
+    by one rounding per entry), same iteration count; with vals_lo = 0 it is the one-word run bit for bit."""
+    import oracle
+    s = tomogen.System(0)
+    f = s.factored()
+    rp, ci, va, lo = factored.expand_exact(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                                           f["sptr"], f["sidx"], f["svals"])
+    m, n = s.dims.m, s.dims.n
+    b = s.rhs(0)
+    o1 = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=30, mode=oracle.DD)
+    o2 = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=30, mode=oracle.DD, vals_lo=lo)
+    o0 = oracle.lsqr(m, n, rp, ci, va, b, damp=s.damp, max_iters=30, mode=oracle.DD, vals_lo=np.zeros_like(va))
+    assert np.array_equal(o0.x, o1.x)
+    assert o2.itn == o1.itn == 30 and not np.array_equal(o2.x, o1.x)
+    assert np.linalg.norm(o2.x - o1.x) <= 1e-11 * np.linalg.norm(o1.x)
