@@ -145,7 +145,10 @@ def workload_config(s, args, iterations_per_step: int, world: int = 1) -> dict:
     vbytes = 4 if args.vals == "f32" else 8
     ab = algorithmic_bytes(m, n, nnz, vbytes) if nrhs == 1 else block_bytes(m, n, nnz, nrhs, vbytes)
     return {"workload": workload_name(s), "iterations_per_step": iterations_per_step,
-            "accumulate": "dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)",
+            "accumulate": ("dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)") +
+                          (("; factored operator with exact entries W*g, depth contraction first (two_stage=2)" if args.accumulate else
+                            "; depth contraction first (two_stage)") if getattr(args, "factored", 0) and
+                           (getattr(args, "two_stage", 1) == 2 or (not args.accumulate and getattr(args, "two_stage", 1) >= 1)) else ""),
             "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
             "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
             "index": ("none: factored operator (lateral footprint x depth kernel, tomo_lsqr_create_factored)" if getattr(args, "factored", 0)
@@ -240,6 +243,8 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
     torch.cuda.synchronize()
     create_wall_ms = 1e3 * (time.perf_counter() - t0)
     S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=0 if factored else args.compress)
+    if factored:
+        S.set(two_stage=getattr(args, "two_stage", 1))
     if args.row_cost is not None:
         S.set(row_cost=args.row_cost)
     if args.pdl is not None:
@@ -293,6 +298,7 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
     out = {"m": m, "n": n, "nnz": nnz, "nrhs": nrhs, "vbytes": vbytes, "create_wall_ms": create_wall_ms, "accumulate": args.accumulate,
            "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms")}
     if factored:
+        out["two_stage"] = getattr(args, "two_stage", 1)
         out["factored"] = {"lateral_entries": S.info("lateral_entries"), "operator_bytes": S.info("operator_bytes"),
                            "cut_nodes_pieces": S.info("cut_nodes_pieces")}
         if torch.cuda.mem_get_info()[0] > 14 * nnz + (2 << 30):
@@ -435,9 +441,20 @@ def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
         # arithmetic.  Work per nonzero and product, in fp64 lane-instructions (an FMA counts once): dd 11 = the value
         # fl(W g) 1 + TwoProd 2 + TwoSum 6 + 2 error adds; fast 2 = the value + the FMA.  Peak as for the dd block solve.
         per = 11.0 if r.get("accumulate", 1) == 1 else 2.0
+        two = r.get("two_stage", 1)
+        contracted = (two == 2) if r.get("accumulate", 1) == 1 else (two >= 1)
         sm_max = (r.get("clocks") or {}).get("sm_max_mhz") or 1965.0
         peak_t = 148 * 64 * sm_max * 1e6 / 1e12
         ach_t = per * nnz * 2 / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e12
+        if contracted:
+            # two-stage contraction: the products per launch are entries x periods (+ the tiny depth stage), klen times fewer
+            # than nonzeros; the kernels are bound by instruction issue and load latency around one (fast) or two (dd) products
+            # per lane and step, so no pipe roofline is claimed: the line reports times only
+            return {"bound": "alu", "kernel": "k_fac2_stage + k_fac2_rows (K1) / k_fac2_cols (K2): depth contraction per node, then W",
+                    "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None, "traffic": None,
+                    "note": "latency / issue bound: klen times fewer products than nonzeros; no roofline claim",
+                    "operator_bytes_per_product": r["factored"]["operator_bytes"],
+                    "k1_us": r["k1_us"], "k2_us": r["k2_us"], "k4_us": r["k4_us"]}
         return {"bound": "alu", "kernel": "k_fac_rows (K1) / k_fac_cols (K2): the two products of an iteration on the factored operator",
                 "achieved": ach_t, "peak": peak_t, "unit": "TFLOP/s", "frac": ach_t / peak_t,
                 "peak_source": "derived: 148 SMs x 64 fp64 lanes/clk x sm_max_mhz (fp64 lane-instructions/s, FMA counted once)",
@@ -522,6 +539,14 @@ def run_ours(args) -> dict | None:
                                        "other_mode": rfac.get("other"), "ms_per_step": rfac["ms"] / args.steps,
                                        "k1_us": rfac["k1_us"], "k2_us": rfac["k2_us"], "k4_us": rfac["k4_us"], "roofline": rff,
                                        "create_ms": rfac["create_ms"], "clocks": rfac["clocks"], **rfac["factored"]}
+        # ... and with the depth contraction first in dd mode too (exact entries W*g, its own oracle: DESIGN.md F-fac3)
+        fx = copy.copy(fa)
+        fx.two_stage = 2
+        rfx = measure(tl, torch, s, fx, barrier, None, 1, args.steps, args.warmup, e2e=False, both_modes=False)
+        also["configs[1] factored, exact entries (two_stage=2)"] = {
+            "workload": workload_name(s), "operator": "factored, entries W*g unrounded, depth contraction per node first; bitwise its own dd oracle",
+            "value": rfx["its"] / (rfx["ms"] * 1e-3), "unit": UNIT, "accumulate": args.accumulate, "ms_per_step": rfx["ms"] / args.steps,
+            "k1_us": rfx["k1_us"], "k2_us": rfx["k2_us"], "k4_us": rfx["k4_us"], "clocks": rfx["clocks"]}
 
     if rank != 0:
         if dist is not None:
@@ -621,6 +646,9 @@ def main():
     ap.add_argument("--vals", default="f64", choices=["f64", "f32"], help="storage type of the matrix values")
     ap.add_argument("--compress", type=int, default=0, choices=[0, 1], help="1: run-compressed index (NEXT-2), reported with its own byte count")
     ap.add_argument("--factored", type=int, default=0, choices=[0, 1], help="1: the factored operator (NEXT-2, second form), reported against the fp64 pipe")
+    ap.add_argument("--two-stage", dest="two_stage", type=int, default=1, choices=[0, 1, 2],
+                    help="factored operator: 0 per-entry products in both modes, 1 (default) depth contraction first in fast mode, "
+                         "2 also in dd mode (exact entries W*g, DESIGN.md F-fac3)")
     ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
     ap.add_argument("--pdl", type=int, default=None, choices=[0, 1], help="tuning: programmatic dependent launch between the kernels of an iteration")
     ap.add_argument("--shards", type=int, default=0, help="NEXT-3: P row blocks solved by tomo_lsqr_solve_sharded (one GPU: all blocks local; torchrun: one block per rank)")

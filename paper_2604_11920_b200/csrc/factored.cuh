@@ -472,8 +472,12 @@ namespace tomo {
 // one rounding per entry, which is inside what "fast" claims (plain fp64 sums, any association; DESIGN.md F-fac2).
 // dd mode never takes this path: its bit-for-bit contract is on the rounded entries.
 // ------------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const double* __restrict__ x, double* __restrict__ S, const Scalars* sc,
-                                                    int check_stop) {
+template <int MODE> struct Fac2S { using type = double; };
+template <> struct Fac2S<1> { using type = double2; };   // dd: S[k, p] and T[k, p] stay unrounded (hi, lo) pairs
+
+template <int MODE>
+__global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const double* __restrict__ x, typename Fac2S<MODE>::type* __restrict__ S,
+                                                    const Scalars* sc, int check_stop) {
   grid_dependency_wait();
   if (check_stop && sc->stop) return;
   const int64_t total = d.nnodes * d.nper;
@@ -482,9 +486,10 @@ __global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const doubl
     const int p = (int)(i - k * d.nper);
     const double* xp = x + k * d.nz + d.kj0[p];
     const double* kp = d.kern + (size_t)p * d.klen;
-    double s = 0.0;
-    for (int t = 0; t < d.klen; ++t) s = fma(kp[t], xp[t], s);
-    S[i] = s;
+    Acc<MODE> s;
+    s.zero();
+    for (int t = 0; t < d.klen; ++t) s.mac(kp[t], xp[t]);
+    if constexpr (MODE == 0) S[i] = s.value(); else S[i] = s.pack();
   }
   grid_launch_dependents();
 }
@@ -493,7 +498,7 @@ __global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const doubl
 // The entries go by in coalesced batches of SB = 32 / G steps (lane l loads entry l of the batch, one batch ahead; the
 // groups pick theirs up by shuffle), the gathers of U steps are in flight before they are used.  (Issuing the next
 // batch's gathers before the current batch is consumed was measured slower: 9.0 k -> 7.6 k it/s at config 1.)
-template <int U, typename GATHER, typename USE>
+template <int U, typename VT, typename GATHER, typename USE>
 __device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const double* __restrict__ val, int64_t e0, int64_t e1, int G, int g,
                                           bool active, int lane, GATHER gather, USE use) {
   const int SB = 32 / G, BE = SB * G;
@@ -508,7 +513,8 @@ __device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const
     double wn = 0.0;
     if (lane < BE && en + lane < e1) { in = idx[en + lane]; wn = val[en + lane]; }
     for (int st = 0; st * G < nb; st += U) {
-      double xs[U], ws[U];
+      VT xs[U];
+      double ws[U];
       bool ok[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
@@ -516,7 +522,7 @@ __device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const
         ok[u] = active && src < nb;
         const int i = __shfl_sync(0xffffffffu, ireg, src & 31);
         ws[u] = __shfl_sync(0xffffffffu, wreg, src & 31);
-        xs[u] = ok[u] ? gather(i) : 0.0;
+        xs[u] = ok[u] ? gather(i) : VT{};
       }
 #pragma unroll
       for (int u = 0; u < U; ++u)
@@ -526,9 +532,9 @@ __device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const
   }
 }
 
-template <int OP>   // OP_PLAIN, OP_K1
+template <int MODE, int OP>   // OP_PLAIN, OP_K1
 __global__ void __launch_bounds__(kFacThreads, 1)
-k_fac2_rows(const FacDesc d, const double* __restrict__ S, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
+k_fac2_rows(const FacDesc d, const typename Fac2S<MODE>::type* __restrict__ S, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
   __shared__ double2 s_slots[kFacWarps];
   __shared__ int s_flag;
   constexpr bool K1 = (OP == OP_K1);
@@ -546,7 +552,7 @@ k_fac2_rows(const FacDesc d, const double* __restrict__ S, const double* __restr
     if (sc->stop) return;
     c = -sc->alpha; sy = sc->rbeta;
   }
-  Acc<0> nsq;
+  Acc<MODE> nsq;
   nsq.zero();
   int q_next = (q0 < q1) ? d.pq[q0] : 0;
   for (int i = q0; i < q1; ++i) {
@@ -554,47 +560,52 @@ k_fac2_rows(const FacDesc d, const double* __restrict__ S, const double* __restr
     if (i + 1 < q1) q_next = d.pq[i + 1];
     const int64_t r = (int64_t)q * nper + lane;
     const double yo = (K1 && lane < nper) ? y[r] * sy : 0.0;
-    Acc<0> a;
+    Acc<MODE> a;
     a.zero();
-    fac2_walk<10>(d.lnode, d.lw, d.lptr[q], d.lptr[q + 1], G, g, active, lane,
-                 [&](int k) { return S[(int64_t)k * nper + p]; }, [&](double w, double sv) { a.mac(w, sv); });
+    using SV = typename Fac2S<MODE>::type;
+    fac2_walk<10, SV>(d.lnode, d.lw, d.lptr[q], d.lptr[q + 1], G, g, active, lane,
+                      [&](int k) { return S[(int64_t)k * nper + p]; },
+                      [&](double w, SV sv) {
+                        if constexpr (MODE == 0) a.mac(w, sv);
+                        else { a.mac(w, sv.x); a.mac(w, sv.y); }   // w * (hi + lo): both words as exact products
+                      });
     for (int gg = 1; gg < G; ++gg) {
-      const Acc<0> o = a.down(gg * nper);
+      const Acc<MODE> o = a.down(gg * nper);
       if (g == 0) a.merge(o);
     }
-    if (lane < nper) y[r] = fac_finish<0, K1, K1>(a, c, yo, nsq);
+    if (lane < nper) y[r] = fac_finish<MODE, K1, K1>(a, c, yo, nsq);
   }
   for (int64_t r = x0 + lane; r < x1; r += 32) {
-    Acc<0> a;
+    Acc<MODE> a;
     a.zero();
     for (int64_t e = d.sptr[r]; e < d.sptr[r + 1]; ++e) a.mac(d.sval[e], x[d.sidx[e]]);
     const int64_t ro = d.mdata + r;
     const double yo = K1 ? y[ro] * sy : 0.0;
-    y[ro] = fac_finish<0, K1, K1>(a, c, yo, nsq);
+    y[ro] = fac_finish<MODE, K1, K1>(a, c, yo, nsq);
   }
   if (lane == 0) d.busy[gw] = clock64() - t_start;
   if (!K1) return;
-  lanes_reduce<32, 0>(nsq);
+  lanes_reduce<32, MODE>(nsq);
   if (lane == 0) s_slots[warp] = nsq.pack();
   __syncthreads();
   grid_launch_dependents();
   if (threadIdx.x == 0) {
-    Acc<0> tot = fac_acc_of<0>(s_slots[0]);
-    for (int i = 1; i < nwarp; ++i) tot.merge(fac_acc_of<0>(s_slots[i]));
+    Acc<MODE> tot = fac_acc_of<MODE>(s_slots[0]);
+    for (int i = 1; i < nwarp; ++i) tot.merge(fac_acc_of<MODE>(s_slots[i]));
     __stcg(partials + blockIdx.x, tot.pack());
   }
   if (!fac_ticket(sc, &s_flag)) return;
-  const double total = final_sum<0>(partials, (int)gridDim.x, s_slots);
+  const double total = final_sum<MODE>(partials, (int)gridDim.x, s_slots);
   if (threadIdx.x == 0) {
     tail_k1(sc, total);
     sc->ticket[0] = 0u;
   }
 }
 
-template <int OP>   // OP_PLAIN, OP_K2, OP_K2_INIT
+template <int MODE, int OP>   // OP_PLAIN, OP_K2, OP_K2_INIT
 __global__ void __launch_bounds__(kFacThreads, 1)
 k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y, Scalars* sc, double2* partials) {
-  __shared__ double s_T[kFacWarps][64];   // per warp: [0, 32) the lanes' sums, [32, 64) the node's T[p]
+  __shared__ double2 s_T[kFacWarps][32];   // per warp: the node's T[p] (dd: unrounded pairs)
   __shared__ double2 s_slots[kFacWarps];
   __shared__ int s_kj0[32];
   __shared__ int s_flag;
@@ -604,7 +615,7 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
   const int nper = d.nper, G = d.G, nz = d.nz, klen = d.klen;
   const int p = lane % nper, g = lane / nper;
   const bool active = g < G;
-  double* my = s_T[warp];
+  double2* my = s_T[warp];
   if (threadIdx.x < 32) s_kj0[threadIdx.x] = (threadIdx.x < nper) ? d.kj0[threadIdx.x] : 0;
   const int s0 = d.wseg[gw], s1 = d.wseg[gw + 1];
   __syncthreads();
@@ -628,19 +639,18 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
     const int node = sg.node;
     int64_t xc0 = 0, xc1 = 0;
     if (d.scptr && lane < nz) { const int64_t colp = (int64_t)node * nz + lane; xc0 = d.scptr[colp]; xc1 = d.scptr[colp + 1]; }
-    Acc<0> a;
+    Acc<MODE> a;
     a.zero();
-    fac2_walk<10>(d.cpair, d.cw, sg.e0, sg.e1, G, g, active, lane,
+    fac2_walk<10, double>(d.cpair, d.cw, sg.e0, sg.e1, G, g, active, lane,
                  [&](int q) { const double xe = x[(int64_t)q * nper + p]; return SCALE ? xe * sx : xe; },
                  [&](double w, double us) { a.mac(w, us); });
     for (int gg = 1; gg < G; ++gg) {     // T[p] of this piece in lanes 0 .. nper-1 (groups in index order)
-      const Acc<0> o = a.down(gg * nper);
+      const Acc<MODE> o = a.down(gg * nper);
       if (g == 0) a.merge(o);
     }
     bool closer = sg.nsegs == 1;
-    double T = a.value();
     if (!closer) {    // a cut node: publish this piece's T, the last piece to arrive adds them in slot order
-      if (lane < nper) __stcg(d.seg_part + (size_t)sg.slot * d.pstride + lane, make_double2(T, 0.0));
+      if (lane < nper) __stcg(d.seg_part + (size_t)sg.slot * d.pstride + lane, a.pack());
       __threadfence();
       __syncwarp();
       unsigned int old = 0;
@@ -652,24 +662,29 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
         if (lane == 0) d.node_cnt[node] = 0u;
         if (lane < nper) {
           const double2* base = d.seg_part + (size_t)(sg.slot - sg.rank) * d.pstride + lane;
-          T = __ldcg(base).x;
-          for (int r = 1; r < sg.nsegs; ++r) T = T + __ldcg(base + (size_t)r * d.pstride).x;
+          a.unpack(__ldcg(base));
+          for (int r = 1; r < sg.nsegs; ++r) a.merge(fac_acc_of<MODE>(__ldcg(base + (size_t)r * d.pstride)));
         }
       }
     }
     if (closer) {
-      if (lane < nper) my[32 + lane] = T;
+      if (lane < nper) my[lane] = a.pack();
       __syncwarp();
-      Acc<0> nsq;
+      Acc<MODE> nsq;
       nsq.zero();
       for (int j = lane; j < nz; j += 32) {
         const int64_t col = (int64_t)node * nz + j;
         const double yo = AXPY ? y[col] : 0.0;
-        Acc<0> S;
+        Acc<MODE> S;
         S.zero();
         for (int pp = 0; pp < nper; ++pp) {     // the depth contraction: periods ascending
           const int t = j - s_kj0[pp];
-          if (t >= 0 && t < klen) S.mac(d.kern[(size_t)pp * klen + t], my[32 + pp]);
+          if (t >= 0 && t < klen) {
+            const double gk = d.kern[(size_t)pp * klen + t];
+            const double2 Tp = my[pp];
+            S.mac(gk, Tp.x);
+            if (MODE == 1) S.mac(gk, Tp.y);   // g * (hi + lo): both words as exact products
+          }
         }
         if (d.scptr) {
           const int64_t c0 = (j == lane) ? xc0 : d.scptr[col], c1 = (j == lane) ? xc1 : d.scptr[col + 1];
@@ -689,10 +704,10 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
               if (base + i < c1) S.mac(vv[i], SCALE ? xe[i] * sx : xe[i]);
           }
         }
-        y[col] = fac_finish<0, AXPY, NORM>(S, c, yo, nsq);
+        y[col] = fac_finish<MODE, AXPY, NORM>(S, c, yo, nsq);
       }
       if (NORM) {
-        lanes_reduce<32, 0>(nsq);
+        lanes_reduce<32, MODE>(nsq);
         if (lane == 0) __stcg(d.node_nsq + node, nsq.pack());
       }
     }
@@ -704,7 +719,7 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
   __syncthreads();
   grid_launch_dependents();
   if (!fac_ticket(sc, &s_flag)) return;
-  const double total = final_sum<0>(d.node_nsq, (int)d.nnodes, s_slots);
+  const double total = final_sum<MODE>(d.node_nsq, (int)d.nnodes, s_slots);
   if (threadIdx.x == 0) {
     if (OP == OP_K2) tail_k2(sc, total);
     if (OP == OP_K2_INIT) tail_init_v(sc, total);

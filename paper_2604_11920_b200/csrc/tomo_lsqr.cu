@@ -72,7 +72,7 @@ struct Dir {
 struct FacState {
   FacDesc d = {};                 // the kernel argument (borrowed W / A_extra CSR arrays, owned rest)
   FacDesc dm[3];                  // ... per mode (0 fast, 1 dd, 2 fast two-stage): the A^T x work split differs (wseg, seg)
-  double* S2 = nullptr;           // two-stage fast mode: S[k, p], the depth contraction of x per node and period
+  double2* S2 = nullptr;          // two-stage contraction: S[k, p], the depth contraction of x per node and period (fast: doubles, dd: pairs)
   int64_t E = 0, snnz = 0;        // lateral entries, entries of the extra rows
   int klp = 0; bool guard = false;  // kernel shape: window length as a template constant (8, 12, 16) or the general one (32, guarded)
   int nsegs = 0, nslots = 0;
@@ -247,10 +247,12 @@ cudaError_t launch_fac_mode(const tomo_lsqr_s* h, bool cols, const double* x, do
     default: return launch_fac_one<MODE, OP, 32, true>(h, cols, x, y, st);
   }
 }
-// fast mode, two-stage contraction (k_fac2_*): the depth contraction once per node, then W
-template <int OP>
+// two-stage contraction (k_fac2_*): the depth contraction once per node, then W.  Fast mode by default; dd mode with
+// option "two_stage" = 2 (exact entries W*g, reading F-fac3)
+template <int MODE, int OP>
 cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double* y, cudaStream_t st) {
   const FacState* f = h->fac;
+  using SV = typename Fac2S<MODE>::type;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -259,23 +261,23 @@ cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double
   cfg.blockDim = dim3(kFacThreads); cfg.gridDim = dim3((unsigned)h->sms);
   if (cols) {
     if constexpr (OP == OP_PLAIN || OP == OP_K2 || OP == OP_K2_INIT)
-      return cudaLaunchKernelEx(&cfg, k_fac2_cols<OP>, f->dm[2], x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac2_cols<MODE, OP>, f->dm[2], x, y, h->sc, h->part_spmv);
   } else {
     if constexpr (OP == OP_PLAIN || OP == OP_K1) {
       cudaLaunchConfig_t c1 = cfg;
       c1.blockDim = dim3(256);
       c1.gridDim = dim3((unsigned)std::max<int64_t>(1, std::min<int64_t>((f->d.nnodes * f->d.nper + 255) / 256, (int64_t)h->sms * 8)));
-      cudaError_t e = cudaLaunchKernelEx(&c1, k_fac2_stage, f->dm[2], x, f->S2, (const Scalars*)h->sc, OP == OP_K1 ? 1 : 0);
+      cudaError_t e = cudaLaunchKernelEx(&c1, k_fac2_stage<MODE>, f->dm[2], x, (SV*)f->S2, (const Scalars*)h->sc, OP == OP_K1 ? 1 : 0);
       if (e != cudaSuccess) return e;
-      return cudaLaunchKernelEx(&cfg, k_fac2_rows<OP>, f->dm[2], (const double*)f->S2, x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac2_rows<MODE, OP>, f->dm[2], (const SV*)f->S2, x, y, h->sc, h->part_spmv);
     }
   }
   return cudaErrorInvalidValue;
 }
 template <int OP>
 void launch_fac(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
-  if (h->accumulate) launch_fac_mode<1, OP>(h, transpose, x, y, st);
-  else if (h->two_stage) launch_fac2<OP>(h, transpose, x, y, st);
+  if (h->accumulate) { if (h->two_stage == 2) launch_fac2<1, OP>(h, transpose, x, y, st); else launch_fac_mode<1, OP>(h, transpose, x, y, st); }
+  else if (h->two_stage) launch_fac2<0, OP>(h, transpose, x, y, st);
   else launch_fac_mode<0, OP>(h, transpose, x, y, st);
 }
 // the > 48 KB dynamic shared memory opt-in of the k_fac_cols instantiations on the current device
@@ -798,7 +800,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     }
     if (rc != TOMO_OK) break;
     ALLOC(f->seg_part, sizeof(double2) * (size_t)std::max(nslots_max, 1) * std::max<int>(nz, nper));
-    ALLOC(f->S2, sizeof(double) * nnodes * nper);
+    ALLOC(f->S2, sizeof(double2) * nnodes * nper);
     ALLOC(f->node_cnt, sizeof(unsigned int) * nnodes); ALLOC(f->node_nsq, sizeof(double2) * nnodes);
     ALLOC(f->busy, sizeof(long long) * NW);
     if ((e = cudaMemsetAsync(f->busy, 0, sizeof(long long) * NW, st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
@@ -982,7 +984,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
       }
       CK(cudaGetLastError());
     }
-    h->kernels_enqueued += (h->fac && !h->accumulate && h->two_stage ? 4.0 : 3.0) * k;   // the two-stage A x is two launches
+    h->kernels_enqueued += (h->fac && (h->accumulate ? h->two_stage == 2 : h->two_stage != 0) ? 4.0 : 3.0) * k;   // the two-stage A x is two launches
     // host poll: {itn, istop, stop}.  The next replay is enqueued before this one is inspected, so the
     // device never idles on the host; kernels after a stop return at once and leave x frozen.
     CK(cudaMemcpyAsync(&h->h_poll[slot], &h->sc->itn, sizeof(PollWord), cudaMemcpyDeviceToHost, st));
@@ -1538,7 +1540,7 @@ extern "C" tomo_status_t tomo_lsqr_set_option(tomo_lsqr_t h, const char* key, in
   else if (k == "accumulate") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->accumulate = (int)value; }
   else if (k == "graph") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->use_graph = (int)value; }
   else if (k == "profile") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->profile = (int)value; }
-  else if (k == "two_stage") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->two_stage = (int)value; }
+  else if (k == "two_stage") { if (value < 0 || value > 2) return TOMO_ERR_INVALID_ARG; h->two_stage = (int)value; }
   else if (k == "multi_shared") { if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG; h->multi_shared = (int)value; }
   else if (k == "compress") {
     if (value != 0 && value != 1) return TOMO_ERR_INVALID_ARG;

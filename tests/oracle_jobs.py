@@ -29,10 +29,18 @@ def _available_ram() -> float:
 
 
 def _run(cfg: int, rhs: int, mode: int, damp: float, atol: float, btol: float, max_iters: int, snapshots: tuple,
-         f32_values: bool = False, solver: str = "lsqr"):
+         f32_values: bool = False, solver: str = "lsqr", exact_entries: bool = False):
     import oracle
     import tomogen
     s = tomogen.System(cfg)
+    if exact_entries:  # the factored operator with exact entries W*g as two-word values (oracle/factored.py expand_exact)
+        from oracle import factored as ofac
+        f = s.factored()
+        rp, ci, va, lo = ofac.expand_exact(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                                           f["sptr"], f["sidx"], f["svals"])
+        r = oracle.lsqr(s.dims.m, s.dims.n, rp, ci, va, s.rhs(rhs), damp=damp, atol=atol, btol=btol, max_iters=max_iters, mode=mode,
+                        snapshots=snapshots, vals_lo=lo)
+        return dict(x=r.x, itn=r.itn, istop=r.istop, r2hist=r.r2norm_hist, snapshots=r.snapshots)
     need = 13.0 * s.dims.nnz + 64.0 * (s.dims.m + s.dims.n)  # CSR (12 B/nnz) + vectors + slack
     if cfg == 2 and _available_ram() < need + 8e9:
         return dict(skipped=f"host RAM: {_available_ram() / 1e9:.0f} GB available, the config-2 CSR needs {need / 1e9:.0f} GB")
@@ -63,6 +71,8 @@ def _all_jobs():
         ("cfg1_dd_f32_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), True),
         # config 1 by LSMR (NEXT-1)
         ("cfg1_lsmr_dd_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (), False, "lsmr"),
+        # config 1 through the factored operator with exact entries (two-stage dd mode, DESIGN.md F-fac3)
+        ("cfg1_ddx_50",): (1, 0, oracle.DD, d1, 0.0, 0.0, 50, (10,), False, "lsqr", True),
         # config 4: skewed system, 100 iterations with x_50 as a snapshot
         ("cfg4_dd_100",): (4, 0, oracle.DD, d4, 0.0, 0.0, 100, (50,)),
         # config 2 (3.7e9 nnz): x_5 of the dd oracle at full size (~45 GB of host RAM, ~25 s per iteration)

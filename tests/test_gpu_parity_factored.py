@@ -43,6 +43,11 @@ def make(tl, f):
                                 dev(f["kj0"].astype(np.int32)), dev(f["kern"]), dev(f["sptr"]), dev(f["sidx"]), dev(f["svals"]))
 
 
+def expand_exact(f):
+    return ofac.expand_exact(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                             f["sptr"], f["sidx"], f["svals"])
+
+
 def expand(f):
     return ofac.expand(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
                        f["sptr"], f["sidx"], f["svals"])
@@ -347,3 +352,56 @@ def test_assemble_csr_configs_and_roundtrip(tl, cfg0):
                                  dev(f["kj0"]), dev(f["kern"]), len(f["sptr"]) - 1, len(f["sidx"]), dev(f["sptr"]), dev(f["sidx"]),
                                  dev(f["svals"]), 7, rp, ci, va)
     assert ei.value.status == T.TOMO_ERR_INVALID_ARG
+
+
+# ---- dd mode on the exact entries W*g (option two_stage = 2; reading F-fac3) ------------------------------
+@pytest.mark.parametrize("shape", SHAPES)
+def test_factored_exact_entries_dd_random_shapes(tl, shape):
+    """The two-stage contraction in dd mode applies the operator with UNROUNDED entries W*g; its oracle is the dd oracle on
+    the two-word entries (oracle/factored.py expand_exact), each sum of exact products rounded once: bitwise."""
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=3000 + npairs, ms=ms, max_entries=60)
+    rp, ci, va, lo = expand_exact(f)
+    m, n = len(rp) - 1, nnodes * nz
+    S = make(tl, f)
+    S.set(accumulate=1, two_stage=2)
+    rng = np.random.default_rng(shape[0] + 1)
+    x, u = rng.standard_normal(n), rng.standard_normal(m)
+    y = S.spmv(dev(x)).cpu().numpy()
+    yt = S.spmv(dev(u), transpose=True).cpu().numpy()
+    assert np.array_equal(y, oracle.spmv(m, n, rp, ci, va, x, oracle.DD, vals_lo=lo))
+    assert np.array_equal(yt, oracle.spmv_t(m, n, rp, ci, va, u, oracle.DD, vals_lo=lo))
+    b = rng.standard_normal(m)
+    xg, res = S.solve(dev(b), damp=0.1, max_iters=20)
+    o = oracle.lsqr(m, n, rp, ci, va, b, damp=0.1, max_iters=20, mode=oracle.DD, vals_lo=lo)
+    assert (res.itn, res.istop) == (o.itn, o.istop) and np.array_equal(xg.cpu().numpy(), o.x)
+    S.set(two_stage=1)   # back on the rounded entries: the CSR bits again
+    x1, _ = S.solve(dev(b), damp=0.1, max_iters=20)
+    assert np.array_equal(x1.cpu().numpy(), oracle.lsqr(m, n, rp, ci, va, b, damp=0.1, max_iters=20, mode=oracle.DD).x)
+    S.close()
+
+
+def test_factored_exact_entries_dd_cfg0_cfg1(tl, cfg0, big):
+    s = cfg0["sys"]
+    f = s.factored()
+    rp, ci, va, lo = expand_exact(f)
+    S = make(tl, f)
+    S.set(accumulate=1, two_stage=2)
+    b = cfg0["b"]
+    xg, res, r2, ar = S.solve(dev(b), damp=s.damp, max_iters=50, history=True)
+    o = oracle.lsqr(cfg0["m"], cfg0["n"], rp, ci, va, b, damp=s.damp, max_iters=50, mode=oracle.DD, vals_lo=lo)
+    assert res.itn == o.itn == 50 and np.array_equal(xg.cpu().numpy(), o.x) and np.array_equal(r2, o.r2norm_hist)
+    x2, _ = S.solve(dev(b), damp=s.damp, max_iters=50)
+    assert torch.equal(xg, x2)
+    S.close()
+    # config 1: x_10 and x_50 against the background run of the exact-entries oracle
+    s1, S1 = big[1]
+    S1.set(accumulate=1, two_stage=2)
+    b1 = dev(s1.rhs(0))
+    o1 = oracle_jobs.get("cfg1_ddx_50")
+    x10, _ = S1.solve(b1, damp=s1.damp, max_iters=10)
+    x50, res = S1.solve(b1, damp=s1.damp, max_iters=50)
+    S1.set(two_stage=1)
+    assert res.itn == 50
+    assert rel(x50.cpu().numpy(), o1["x"]) <= TOL_X50 and np.array_equal(x10.cpu().numpy(), o1["snapshots"][10])
+    assert np.array_equal(x50.cpu().numpy(), o1["x"])
