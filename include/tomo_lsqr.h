@@ -212,12 +212,17 @@ tomo_status_t tomo_lsqr_get_csc(tomo_lsqr_t h, int64_t* d_colptr, int32_t* d_row
  *                          ordering of PAPER.md Eq. 7 P:79 makes every lateral node of a ray a run of consecutive
  *                          columns, Eq. 5) and streams those instead of the int32 arrays.  Same elements,
  *                          same order: results are bitwise those of "compress" = 0.  Default 0.
- *   "two_stage"   0 | 1    factored handles, "accumulate" = 0 only (default 1): apply A_data as W after the depth contraction
+ *   "two_stage"   0 | 1 | 2  factored handles (default 1: in fast mode only): apply A_data as W after the depth contraction
  *                          S[k, p] = sum_t g_p[t] x[k nz + j0_p + t] (and A_data^T as the contraction of T[k, p] = sum_q W[q, k]
  *                          u[q nper + p]): klen times fewer products.  The operator applied has the UNROUNDED entries W g
  *                          (one rounding per entry away from the CSR form's fl(W g)); results stay within the fast-mode
  *                          bar (SpMV 1e-12, x_k as any other summation order).  0: per-entry products of the rounded values.
- *                          Never used with "accumulate" = 1, whose results are bit for bit those of the CSR form.
+ *                          With 0 and 1, "accumulate" = 1 works on the rounded entries and its results are bit for bit
+ *                          those of the CSR form.  2: the contraction in dd mode too.  S and T are kept as unrounded
+ *                          (hi, lo) pairs, every product of both words is exact and each result is rounded ONCE: the
+ *                          order-independent iterate of the operator with EXACT entries W g (Eq. 5 in real
+ *                          arithmetic; reading F-fac3), bit for bit the dd oracle on two-word entries
+ *                          (oracle/factored.py expand_exact) and ~1e-13 away from the CSR form's x_k.
  *   "pdl"         0 | 1    chain the kernels of an iteration with programmatic dependent launch (default 1): the
  *                          prologue of a kernel (barrier set-up, split points, first bulk copies) overlaps the
  *                          tail of the previous one; never changes results
