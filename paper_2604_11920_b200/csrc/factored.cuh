@@ -555,19 +555,32 @@ k_fac2_rows(const FacDesc d, const typename Fac2S<MODE>::type* __restrict__ S, c
   Acc<MODE> nsq;
   nsq.zero();
   int q_next = (q0 < q1) ? d.pq[q0] : 0;
+  int64_t en0 = 0, en1 = 0;
+  if (q0 < q1) { en0 = d.lptr[q_next]; en1 = d.lptr[q_next + 1]; }
+  int q_next2 = (q0 + 1 < q1) ? d.pq[q0 + 1] : 0;
   for (int i = q0; i < q1; ++i) {
     const int q = q_next;
-    if (i + 1 < q1) q_next = d.pq[i + 1];
+    const int64_t pe0 = en0, pe1 = en1;
+    q_next = q_next2;
+    if (i + 1 < q1) { en0 = d.lptr[q_next]; en1 = d.lptr[q_next + 1]; }   // the next pair's range and the pair after it
+    if (i + 2 < q1) q_next2 = d.pq[i + 2];
     const int64_t r = (int64_t)q * nper + lane;
     const double yo = (K1 && lane < nper) ? y[r] * sy : 0.0;
     Acc<MODE> a;
     a.zero();
     using SV = typename Fac2S<MODE>::type;
-    fac2_walk<10, SV>(d.lnode, d.lw, d.lptr[q], d.lptr[q + 1], G, g, active, lane,
+    fac2_walk<10, SV>(d.lnode, d.lw, pe0, pe1, G, g, active, lane,
                       [&](int k) { return S[(int64_t)k * nper + p]; },
                       [&](double w, SV sv) {
                         if constexpr (MODE == 0) a.mac(w, sv);
-                        else { a.mac(w, sv.x); a.mac(w, sv.y); }   // w * (hi + lo): both words as exact products
+                        else {   // w * (hi + lo): TwoProd of the high word, the low word's product joins its error term
+                          const double pr = w * sv.x;
+                          const double er = fma(w, sv.y, fma(w, sv.x, -pr));
+                          double sm, qq;
+                          two_sum(a.v.hi, pr, sm, qq);
+                          a.v.hi = sm;
+                          a.v.lo = a.v.lo + (qq + er);
+                        }
                       });
     for (int gg = 1; gg < G; ++gg) {
       const Acc<MODE> o = a.down(gg * nper);

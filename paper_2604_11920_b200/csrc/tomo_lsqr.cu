@@ -71,7 +71,7 @@ struct Dir {
 // the factored sensitivity block (factored.cuh; tomo_lsqr_create_factored): what the handle owns of it
 struct FacState {
   FacDesc d = {};                 // the kernel argument (borrowed W / A_extra CSR arrays, owned rest)
-  FacDesc dm[3];                  // ... per mode (0 fast, 1 dd, 2 fast two-stage): the A^T x work split differs (wseg, seg)
+  FacDesc dm[4];                  // ... per mode (0 fast, 1 dd, 2 fast two-stage, 3 dd two-stage): the A^T x work split differs (wseg, seg)
   double2* S2 = nullptr;          // two-stage contraction: S[k, p], the depth contraction of x per node and period (fast: doubles, dd: pairs)
   int64_t E = 0, snnz = 0;        // lateral entries, entries of the extra rows
   int klp = 0; bool guard = false;  // kernel shape: window length as a template constant (8, 12, 16) or the general one (32, guarded)
@@ -79,7 +79,7 @@ struct FacState {
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
-  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[3] = {nullptr, nullptr, nullptr}; FacSeg* seg[3] = {nullptr, nullptr, nullptr};
+  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[4] = {nullptr, nullptr, nullptr, nullptr}; FacSeg* seg[4] = {nullptr, nullptr, nullptr, nullptr};
   double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
 };
 
@@ -261,7 +261,7 @@ cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double
   cfg.blockDim = dim3(kFacThreads); cfg.gridDim = dim3((unsigned)h->sms);
   if (cols) {
     if constexpr (OP == OP_PLAIN || OP == OP_K2 || OP == OP_K2_INIT)
-      return cudaLaunchKernelEx(&cfg, k_fac2_cols<MODE, OP>, f->dm[2], x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac2_cols<MODE, OP>, f->dm[MODE ? 3 : 2], x, y, h->sc, h->part_spmv);
   } else {
     if constexpr (OP == OP_PLAIN || OP == OP_K1) {
       cudaLaunchConfig_t c1 = cfg;
@@ -500,7 +500,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
     cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
-    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->S2); for (int i = 0; i < 3; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->S2); for (int i = 0; i < 4; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
     cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
   }
@@ -732,10 +732,10 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     std::vector<int64_t> cptr((size_t)nnodes + 1);
     if ((e = cudaMemcpyAsync(cptr.data(), f->cptr, sizeof(int64_t) * (nnodes + 1), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the node pointers"); break; }
-    std::vector<FacSeg> segs_m[3];
-    std::vector<int32_t> wseg_m[3];
+    std::vector<FacSeg> segs_m[4];
+    std::vector<int32_t> wseg_m[4];
     int nslots_max = 0;
-    for (int mode = 0; mode < 3; ++mode) {
+    for (int mode = 0; mode < 4; ++mode) {
       std::vector<FacSeg>& segs = segs_m[mode];
       std::vector<int32_t>& wseg = wseg_m[mode];
       std::vector<int32_t> owner;
@@ -746,7 +746,8 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       // measured on B200 (per-warp busy cycles): closing a node is a chain of dependent loads worth ~5 k cycles,
       // i.e. the time of ~26 entries in dd mode and ~55 in fast mode, hence one split per mode
       // (two-stage fast mode: an entry is one FMA, the closing is the same chain: ~250 entries)
-      const double kClose = mode == 1 ? 26.0 : mode == 0 ? 55.0 : 250.0, kCloseEmpty = mode == 1 ? 14.0 : mode == 0 ? 28.0 : 125.0;
+      const double kCloseM[4] = {55.0, 26.0, 250.0, 110.0};
+      const double kClose = kCloseM[mode], kCloseEmpty = 0.5 * kCloseM[mode];
       const int64_t kMinPiece = 8;
       int64_t empty = 0;
       for (int64_t k = 0; k < nnodes; ++k) empty += cptr[k] == cptr[k + 1];
@@ -791,7 +792,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     }
     ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->pq, sizeof(int32_t) * npairs);
     if ((e = cudaMemcpyAsync(f->pq, pq.data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the pair lists"); break; }
-    for (int mode = 0; mode < 3 && rc == TOMO_OK; ++mode) {
+    for (int mode = 0; mode < 4 && rc == TOMO_OK; ++mode) {
       if ((e = cudaMalloc(&f->wseg[mode], sizeof(int32_t) * (NW + 1))) != cudaSuccess ||
           (e = cudaMalloc(&f->seg[mode], sizeof(FacSeg) * std::max<size_t>(segs_m[mode].size(), 1))) != cudaSuccess ||
           (e = cudaMemcpyAsync(f->wseg[mode], wseg_m[mode].data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
@@ -834,7 +835,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     d.pw = f->pw; d.pq = f->pq; d.wseg = f->wseg[1]; d.seg = f->seg[1];
     d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq; d.busy = f->busy;
     d.pstride = std::max<int>(nz, nper);
-    for (int mode = 0; mode < 3; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
+    for (int mode = 0; mode < 4; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
     cudaEventRecord(e1, st);
     if ((e = cudaEventSynchronize(e1)) != cudaSuccess) { rc = cuda_fail(e, "create_factored"); break; }
     float msf = 0;
