@@ -513,20 +513,21 @@ __device__ __forceinline__ void fac2_walk(const int32_t* __restrict__ idx, const
     double wn = 0.0;
     if (lane < BE && en + lane < e1) { in = idx[en + lane]; wn = val[en + lane]; }
     for (int st = 0; st * G < nb; st += U) {
+      // no branch per step: a step beyond the batch takes weight 0 and entry 0 (its product adds an exact zero); the
+      // idle lanes behind the last group sum into accumulators nobody reads
       VT xs[U];
       double ws[U];
-      bool ok[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int src = (st + u) * G + g;
-        ok[u] = active && src < nb;
+        const bool in = src < nb;
         const int i = __shfl_sync(0xffffffffu, ireg, src & 31);
-        ws[u] = __shfl_sync(0xffffffffu, wreg, src & 31);
-        xs[u] = ok[u] ? gather(i) : VT{};
+        const double w = __shfl_sync(0xffffffffu, wreg, src & 31);
+        ws[u] = in ? w : 0.0;
+        xs[u] = gather(in ? i : 0);
       }
 #pragma unroll
-      for (int u = 0; u < U; ++u)
-        if (ok[u]) use(ws[u], xs[u]);
+      for (int u = 0; u < U; ++u) use(ws[u], xs[u]);
     }
     ireg = in; wreg = wn; eb = en;
   }
