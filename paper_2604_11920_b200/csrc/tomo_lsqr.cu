@@ -79,7 +79,7 @@ struct FacState {
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
-  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* wseg[4] = {nullptr, nullptr, nullptr, nullptr}; FacSeg* seg[4] = {nullptr, nullptr, nullptr, nullptr};
+  int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* pw2 = nullptr; int32_t* pq2 = nullptr; int32_t* wseg[4] = {nullptr, nullptr, nullptr, nullptr}; FacSeg* seg[4] = {nullptr, nullptr, nullptr, nullptr};
   double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
 };
 
@@ -267,9 +267,9 @@ cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double
       cudaLaunchConfig_t c1 = cfg;
       c1.blockDim = dim3(256);
       c1.gridDim = dim3((unsigned)std::max<int64_t>(1, std::min<int64_t>((f->d.nnodes * f->d.nper + 255) / 256, (int64_t)h->sms * 8)));
-      cudaError_t e = cudaLaunchKernelEx(&c1, k_fac2_stage<MODE>, f->dm[2], x, (SV*)f->S2, (const Scalars*)h->sc, OP == OP_K1 ? 1 : 0);
+      cudaError_t e = cudaLaunchKernelEx(&c1, k_fac2_stage<MODE>, f->dm[MODE ? 3 : 2], x, (SV*)f->S2, (const Scalars*)h->sc, OP == OP_K1 ? 1 : 0);
       if (e != cudaSuccess) return e;
-      return cudaLaunchKernelEx(&cfg, k_fac2_rows<MODE, OP>, f->dm[2], (const SV*)f->S2, x, y, h->sc, h->part_spmv);
+      return cudaLaunchKernelEx(&cfg, k_fac2_rows<MODE, OP>, f->dm[MODE ? 3 : 2], (const SV*)f->S2, x, y, h->sc, h->part_spmv);
     }
   }
   return cudaErrorInvalidValue;
@@ -500,7 +500,7 @@ void free_handle(tomo_lsqr_s* h) {
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
     cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
-    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->S2); for (int i = 0; i < 4; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
+    cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->pw2); cudaFree(f->pq2); cudaFree(f->S2); for (int i = 0; i < 4; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
     cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
   }
@@ -689,14 +689,18 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
         (e = cudaMemcpyAsync(f->kern, d_kern, sizeof(double) * nper * klen, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "copy of the kernel table"); break; }
     // --- static work split (host): pairs by entry count for A x; lateral-CSC entries cut evenly for A^T x ---
     const int G = 32 / nper;
-    std::vector<int32_t> pw((size_t)NW + 1), pq((size_t)npairs);
-    {
+    std::vector<int32_t> pw_k[2], pq_k[2];
+    for (int kind = 0; kind < 2; ++kind) {   // 0: per-entry kernels, 1: two-stage kernels (a pair's fixed cost weighs 3 steps there)
+      std::vector<int32_t>& pw = pw_k[kind];
+      std::vector<int32_t>& pq = pq_k[kind];
+      pw.assign((size_t)NW + 1, 0); pq.assign((size_t)npairs, 0);
+      const double kPair = kind ? 3.0 : 0.3;
       // cost of a pair in lane steps: ceil(entries / G) + 0.3 (group combine, row stores; fitted to the per-warp busy
       // cycles on B200: 245 cycles per pair against 918 per step in dd mode, 104 against 512 in fast mode).
       // A CTA takes a contiguous run of pairs (equal cost); inside the CTA the pairs are dealt to the warps longest
       // first, each to the least loaded warp (a contiguous split at pair granularity left +-18 % between warps);
       // a warp walks its pairs in ascending order.
-      auto cost = [&](int64_t q) { return (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + 0.3; };
+      auto cost = [&](int64_t q) { return (double)((lptr[q + 1] - lptr[q] + G - 1) / G) + kPair; };
       std::vector<double> pre((size_t)npairs + 1, 0.0);
       for (int64_t q = 0; q < npairs; ++q) pre[q + 1] = pre[q] + cost(q);
       std::vector<int64_t> pc((size_t)sms + 1, 0);
@@ -746,7 +750,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       // measured on B200 (per-warp busy cycles): closing a node is a chain of dependent loads worth ~5 k cycles,
       // i.e. the time of ~26 entries in dd mode and ~55 in fast mode, hence one split per mode
       // (two-stage fast mode: an entry is one FMA, the closing is the same chain: ~250 entries)
-      const double kCloseM[4] = {55.0, 26.0, 250.0, 110.0};
+      const double kCloseM[4] = {55.0, 26.0, 330.0, 160.0};
       const double kClose = kCloseM[mode], kCloseEmpty = 0.5 * kCloseM[mode];
       const int64_t kMinPiece = 8;
       int64_t empty = 0;
@@ -791,7 +795,10 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
       nslots_max = std::max(nslots_max, nslots);
     }
     ALLOC(f->pw, sizeof(int32_t) * (NW + 1)); ALLOC(f->pq, sizeof(int32_t) * npairs);
-    if ((e = cudaMemcpyAsync(f->pq, pq.data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the pair lists"); break; }
+    ALLOC(f->pw2, sizeof(int32_t) * (NW + 1)); ALLOC(f->pq2, sizeof(int32_t) * npairs);
+    if ((e = cudaMemcpyAsync(f->pq, pq_k[0].data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(f->pq2, pq_k[1].data(), sizeof(int32_t) * npairs, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(f->pw2, pw_k[1].data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the pair lists"); break; }
     for (int mode = 0; mode < 4 && rc == TOMO_OK; ++mode) {
       if ((e = cudaMalloc(&f->wseg[mode], sizeof(int32_t) * (NW + 1))) != cudaSuccess ||
           (e = cudaMalloc(&f->seg[mode], sizeof(FacSeg) * std::max<size_t>(segs_m[mode].size(), 1))) != cudaSuccess ||
@@ -805,7 +812,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     ALLOC(f->node_cnt, sizeof(unsigned int) * nnodes); ALLOC(f->node_nsq, sizeof(double2) * nnodes);
     ALLOC(f->busy, sizeof(long long) * NW);
     if ((e = cudaMemsetAsync(f->busy, 0, sizeof(long long) * NW, st)) != cudaSuccess) { rc = cuda_fail(e, "memset"); break; }
-    if ((e = cudaMemcpyAsync(f->pw, pw.data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+    if ((e = cudaMemcpyAsync(f->pw, pw_k[0].data(), sizeof(int32_t) * (NW + 1), cudaMemcpyHostToDevice, st)) != cudaSuccess ||
         (e = cudaMemsetAsync(f->node_cnt, 0, sizeof(unsigned int) * nnodes, st)) != cudaSuccess ||
         (e = cudaMemsetAsync(f->node_nsq, 0, sizeof(double2) * nnodes, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "upload of the work split"); break; }
@@ -835,7 +842,10 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     d.pw = f->pw; d.pq = f->pq; d.wseg = f->wseg[1]; d.seg = f->seg[1];
     d.seg_part = f->seg_part; d.node_cnt = f->node_cnt; d.node_nsq = f->node_nsq; d.busy = f->busy;
     d.pstride = std::max<int>(nz, nper);
-    for (int mode = 0; mode < 4; ++mode) { f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode]; }
+    for (int mode = 0; mode < 4; ++mode) {
+      f->dm[mode] = d; f->dm[mode].wseg = f->wseg[mode]; f->dm[mode].seg = f->seg[mode];
+      if (mode >= 2) { f->dm[mode].pw = f->pw2; f->dm[mode].pq = f->pq2; }
+    }
     cudaEventRecord(e1, st);
     if ((e = cudaEventSynchronize(e1)) != cudaSuccess) { rc = cuda_fail(e, "create_factored"); break; }
     float msf = 0;
