@@ -333,6 +333,7 @@ void launch_k4(const tomo_lsqr_s* h, cudaStream_t st) {
 }
 
 tomo_status_t rebuild_partitions(tomo_lsqr_s* h, cudaStream_t st) {
+  if (h->fac) { h->part_dirty = false; return TOMO_OK; }   // a factored handle has its own static splits (built at create)
   if (!h->part_dirty) return TOMO_OK;
   const int tb = 128;
   // one persistent CTA per SM, W warp ranges each: cost-balanced element split points at multiples of the tile size

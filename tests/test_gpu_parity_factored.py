@@ -163,6 +163,11 @@ def test_factored_edge_cases_and_errors(tl):
     assert res.istop == 0 and res.itn == 0 and not x.any()
     x, res = S.solve(dev(np.ones(m)), damp=0.1, max_iters=0)
     assert res.istop == 7 and res.itn == 0 and not x.any()
+    # an option that only concerns the CSR path is accepted and changes nothing
+    xa, _ = S.solve(dev(np.ones(m)), damp=0.1, max_iters=7)
+    S.set(row_cost=100)
+    xb, _ = S.solve(dev(np.ones(m)), damp=0.1, max_iters=7)
+    assert torch.equal(xa, xb)
     # calls a factored handle does not take
     for call in (lambda: T.tomo_lsqr_update_values(S.h, dev(va)), lambda: S.csc(), lambda: S.set(compress=1)):
         with pytest.raises(T.TomoError) as ei:
