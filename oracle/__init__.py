@@ -47,6 +47,8 @@ def _load():
         lib.oracle_spmv_t_x.restype = None
         lib.oracle_lsqr_solve_x.argtypes = [i64, i64, vp, vp, vp, vp, vp, f64, f64, f64, i32, ci, vp, vp, vp, vp, i32, vp, vp]
         lib.oracle_lsqr_solve_x.restype = None
+        lib.oracle_lsmr_solve_x.argtypes = lib.oracle_lsqr_solve_x.argtypes
+        lib.oracle_lsmr_solve_x.restype = None
         lib.oracle_csr_to_csc.argtypes = [i64, i64, vp, vp, vp, vp, vp, vp]
         lib.oracle_csr_to_csc.restype = None
         lib.oracle_lsqr_new.argtypes = [i64, i64, vp, vp, vp, vp, f64, f64, f64, i32, ci]
@@ -166,9 +168,10 @@ class LsmrResult:
     snapshots: dict
 
 
-def lsmr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, mode=PLAIN, snapshots=()):
-    """Run the oracle LSMR (Fong & Saunders; the paper's own solver)."""
+def lsmr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=50, mode=PLAIN, snapshots=(), vals_lo=None):
+    """Run the oracle LSMR (Fong & Saunders; the paper's own solver).  vals_lo: as in lsqr."""
     rp, ci, va = _csr(rowptr, colind, vals)
+    lo = None if vals_lo is None else np.ascontiguousarray(vals_lo, dtype=np.float64)
     b = np.ascontiguousarray(b, dtype=np.float64)
     assert len(b) == m and len(rp) == m + 1
     x = np.zeros(n, dtype=np.float64)
@@ -177,9 +180,9 @@ def lsmr(m, n, rowptr, colind, vals, b, damp=0.0, atol=0.0, btol=0.0, max_iters=
     narh = np.full(max(max_iters, 1), np.nan)
     snaps = np.ascontiguousarray(sorted(int(k) for k in snapshots), dtype=np.int32)
     sx = np.full((len(snaps), n), np.nan)
-    _load().oracle_lsmr_solve(m, n, _p(rp), _p(ci), _p(va), _p(b), damp, atol, btol, int(max_iters), mode,
-                              _p(x), _p(res), _p(nrh), _p(narh), len(snaps), _p(snaps) if len(snaps) else None,
-                              _p(sx) if len(snaps) else None)
+    _load().oracle_lsmr_solve_x(m, n, _p(rp), _p(ci), _p(va), _p(lo), _p(b), damp, atol, btol, int(max_iters), mode,
+                                _p(x), _p(res), _p(nrh), _p(narh), len(snaps), _p(snaps) if len(snaps) else None,
+                                _p(sx) if len(snaps) else None)
     itn = int(res[0])
     return LsmrResult(x, itn, int(res[1]), res[2], res[3], res[4], res[5], res[6], nrh[:itn].copy(), narh[:itn].copy(),
                       {int(k): sx[i] for i, k in enumerate(snaps)})

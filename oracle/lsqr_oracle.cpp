@@ -491,12 +491,24 @@ void oracle_lsqr_solve_x(int64_t m, int64_t n, const int64_t* rowptr, const int3
 
 // LSMR, whole solve.  res[0..7] = itn, istop, normr, normar, normA, condA, normx, 0.
 // nrhist / narhist: [max_iters] or NULL; snapshots as in oracle_lsqr_solve.
+void oracle_lsmr_solve_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                         const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
+                         double* x, double* res, double* nrhist, double* narhist,
+                         int32_t nsnap, const int32_t* snap_iters, double* snap_x);
 void oracle_lsmr_solve(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals,
                        const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
                        double* x, double* res, double* nrhist, double* narhist,
                        int32_t nsnap, const int32_t* snap_iters, double* snap_x) {
+  oracle_lsmr_solve_x(m, n, rowptr, colind, vals, nullptr, b, damp, atol, btol, max_iters, mode, x, res, nrhist, narhist, nsnap, snap_iters,
+                      snap_x);
+}
+// the same on two-word entries vals + vals_lo (NULL: one-word entries)
+void oracle_lsmr_solve_x(int64_t m, int64_t n, const int64_t* rowptr, const int32_t* colind, const double* vals, const double* vals_lo,
+                         const double* b, double damp, double atol, double btol, int32_t max_iters, int mode,
+                         double* x, double* res, double* nrhist, double* narhist,
+                         int32_t nsnap, const int32_t* snap_iters, double* snap_x) {
   Lsmr* s = new Lsmr();
-  s->A = Csr{m, n, rowptr, colind, vals};
+  s->A = Csr{m, n, rowptr, colind, vals, vals_lo};
   s->mode = mode; s->damp = damp; s->atol = atol; s->btol = btol; s->max_iters = max_iters;
   s->init(b);
   int32_t sn = 0;

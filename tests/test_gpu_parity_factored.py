@@ -398,6 +398,10 @@ def test_factored_exact_entries_dd_cfg0_cfg1(tl, cfg0, big):
     assert res.itn == o.itn == 50 and np.array_equal(xg.cpu().numpy(), o.x) and np.array_equal(r2, o.r2norm_hist)
     x2, _ = S.solve(dev(b), damp=s.damp, max_iters=50)
     assert torch.equal(xg, x2)
+    # LSMR, the paper's own solver, on the exact entries
+    xl, resl = S.solve(dev(b), damp=s.damp, max_iters=50, solver="lsmr")
+    ol = oracle.lsmr(cfg0["m"], cfg0["n"], rp, ci, va, b, damp=s.damp, max_iters=50, mode=oracle.DD, vals_lo=lo)
+    assert resl.itn == ol.itn == 50 and np.array_equal(xl.cpu().numpy(), ol.x)
     S.close()
     # config 1: x_10 and x_50 against the background run of the exact-entries oracle
     s1, S1 = big[1]
