@@ -97,8 +97,8 @@ tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t n
  * with option "two_stage" = 1, the unrounded entries W g).
  * Supported on such a handle: tomo_lsqr_solve / tomo_lsmr_solve, *_solve_host, *_solve_multi (the sides run one after
  * the other), tomo_lsqr_spmv, the options "check_every", "accumulate", "graph", "profile", "pdl", "two_stage", and get_info.
- * Not supported (INVALID_ARG): tomo_lsqr_update_values (nothing is stored per nonzero: create again, it costs
- * milliseconds), tomo_lsqr_get_csc, "compress" = 1, tomo_lsqr_solve_sharded.
+ * Not supported (INVALID_ARG): tomo_lsqr_update_values (nothing is stored per nonzero: tomo_lsqr_update_kernels
+ * replaces the depth kernels), tomo_lsqr_get_csc, "compress" = 1, tomo_lsqr_solve_sharded.
  * Errors: INVALID_ARG, RANGE, NOT_DEVICE_PTR, BAD_CSR (W, A_extra or the kernel table malformed / non-finite),
  * UNSUPPORTED_ARCH, OOM, CUDA; *out is NULL on error. */
 tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz,
@@ -121,6 +121,15 @@ tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, int64_t nnode
                                      const double* d_kern, int64_t ms, int64_t snnz, const int64_t* d_sptr, const int32_t* d_sidx,
                                      const double* d_svals, int64_t nnz, int64_t* d_rowptr, int32_t* d_colind, double* d_vals,
                                      void* cuda_stream);
+
+/* NEXT-4 for a factored handle: new depth kernels on the same rays.  The outer Gauss-Newton loop
+ * re-evaluates the depth kernels of the updated model and solves again; W (the rays' lateral footprints), its transpose
+ * and the work splits stay.  d_kj0 int32[nper], d_kern fp64[nper * klen] (same nper, klen, nz as at create; DEVICE arrays;
+ * copied into the handle: the caller's arrays are not kept).  Costs two small copies.  Results of later solves are
+ * bitwise those of a handle created from scratch with the new table.
+ * Errors: INVALID_ARG (not a factored handle, NULL), NOT_DEVICE_PTR, BAD_CSR (a window outside [0, nz) or a non-finite
+ * value; the handle is unchanged), CUDA. */
+tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream);
 
 /* NEXT-4: value-only refresh.  The outer Gauss-Newton loop of the inversion
  * re-evaluates G on the same rays and solves again: the sparsity pattern, hence the CSC permutation, the split

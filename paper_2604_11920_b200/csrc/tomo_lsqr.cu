@@ -1396,6 +1396,31 @@ tomo_status_t update_values_t(tomo_lsqr_s* h, const VT* d_vals, cudaStream_t st)
 }
 }  // namespace
 
+// NEXT-4 for the factored form: new depth kernels on the same rays
+extern "C" tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream) {
+  if (!h || !h->fac || !d_kj0 || !d_kern) return TOMO_ERR_INVALID_ARG;
+  { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
+  if (!is_device_ptr(d_kj0) || !is_device_ptr(d_kern)) return TOMO_ERR_NOT_DEVICE_PTR;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FacState* f = h->fac;
+  const int nper = f->d.nper, klen = f->d.klen, nz = f->d.nz;
+  int* d_flags = nullptr;
+  CK(cudaMalloc(&d_flags, sizeof(int)));
+  cudaMemsetAsync(d_flags, 0, sizeof(int), st);
+  k_fac_validate_kern<<<1, 256, 0, st>>>(nper, nz, klen, d_kj0, d_kern, d_flags);
+  int flags = 0;
+  cudaError_t e = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_flags);
+  if (e != cudaSuccess) return cuda_fail(e, "validation of the kernel table");
+  if (flags) return TOMO_ERR_BAD_CSR;   // nothing has been touched
+  // the handle's own copies are overwritten in place: captured graphs keep pointing at them
+  CK(cudaMemcpyAsync(f->kj0, d_kj0, sizeof(int32_t) * nper, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(f->kern, d_kern, sizeof(double) * nper * klen, cudaMemcpyDeviceToDevice, st));
+  CK(cudaStreamSynchronize(st));
+  return TOMO_OK;
+}
+
 extern "C" tomo_status_t tomo_lsqr_update_values(tomo_lsqr_t h, const void* d_vals, void* cuda_stream) {
   if (!h || h->fac || (h->nnz > 0 && !d_vals)) return TOMO_ERR_INVALID_ARG;  // a factored handle stores no value per nonzero
   { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }

@@ -414,3 +414,38 @@ def test_factored_exact_entries_dd_cfg0_cfg1(tl, cfg0, big):
     assert res.itn == 50
     assert rel(x50.cpu().numpy(), o1["x"]) <= TOL_X50 and np.array_equal(x10.cpu().numpy(), o1["snapshots"][10])
     assert np.array_equal(x50.cpu().numpy(), o1["x"])
+
+
+def test_update_kernels_equals_create_from_scratch(tl):
+    """NEXT-4 on a factored handle: new depth kernels on the same rays (the outer Gauss-Newton loop, P:77 / P:81);
+    every mode, also after a graph was captured with the old table."""
+    import paper_2604_11920_b200 as T
+    f = tomogen.random_factored(400, 10, 120, 20, 12, seed=91)
+    rng = np.random.default_rng(92)
+    g = dict(f)
+    g["kern"] = rng.standard_normal(f["kern"].shape)
+    g["kj0"] = rng.integers(0, f["nz"] - f["klen"] + 1, size=f["nper"]).astype(np.int32)
+    S, R = make(tl, f), make(tl, g)
+    b = dev(rng.standard_normal(S.m))
+    for acc, ts in ((1, 1), (1, 2), (0, 1), (0, 0)):
+        S.set(accumulate=acc, two_stage=ts)
+        S.solve(b, damp=0.1, max_iters=12)      # captures a graph on the old table (first pass) / the refreshed one (later)
+    T.tomo_lsqr_update_kernels(S.h, dev(g["kj0"]), dev(g["kern"]))
+    for acc, ts in ((1, 1), (1, 2), (0, 1), (0, 0)):
+        S.set(accumulate=acc, two_stage=ts); R.set(accumulate=acc, two_stage=ts)
+        assert torch.equal(S.solve(b, damp=0.1, max_iters=12)[0], R.solve(b, damp=0.1, max_iters=12)[0]), (acc, ts)
+    # and the oracle on the new multiplied-out matrix
+    rp, ci, va = expand(g)
+    S.set(accumulate=1, two_stage=1)
+    o = oracle.lsqr(S.m, S.n, rp, ci, va, b.cpu().numpy(), damp=0.1, max_iters=12, mode=oracle.DD)
+    assert np.array_equal(S.solve(b, damp=0.1, max_iters=12)[0].cpu().numpy(), o.x)
+    # a bad table leaves the handle as it was
+    bad = g["kern"].copy(); bad[0, 0] = np.inf
+    with pytest.raises(T.TomoError) as ei:
+        T.tomo_lsqr_update_kernels(S.h, dev(g["kj0"]), dev(bad))
+    assert ei.value.status == T.TOMO_ERR_BAD_CSR
+    assert np.array_equal(S.solve(b, damp=0.1, max_iters=12)[0].cpu().numpy(), o.x)
+    C = tl.TomoLsqr(S.m, S.n, dev(rp), dev(ci), dev(va))
+    with pytest.raises(T.TomoError):
+        T.tomo_lsqr_update_kernels(C.h, dev(g["kj0"]), dev(g["kern"]))   # not a factored handle
+    C.close(); S.close(); R.close()
