@@ -25,10 +25,13 @@ def expand(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None, sidx
     lptr = np.asarray(lptr, dtype=np.int64)
     lnode = np.asarray(lnode, dtype=np.int64)
     lw = np.asarray(lw, dtype=np.float64)
-    kern = np.asarray(kern, dtype=np.float64).reshape(nper, -1)
-    klen = kern.shape[1]
+    kern = np.asarray(kern, dtype=np.float64)
     kj0 = np.asarray(kj0, dtype=np.int64)
-    assert lptr.shape == (npairs + 1,) and kj0.shape == (nper,)
+    nodal = kern.ndim == 3       # kernel table per lateral node (the paper's Theta_k): kern[k, p, t], kj0[k, p]
+    if not nodal:
+        kern = kern.reshape(nper, -1)
+    klen = kern.shape[-1]
+    assert lptr.shape == (npairs + 1,) and kj0.shape == ((nnodes, nper) if nodal else (nper,))
     assert np.all(kj0 >= 0) and np.all(kj0 + klen <= nz)
     cnt = np.diff(lptr)                                   # lateral entries per pair
     ms = 0 if sptr is None else len(sptr) - 1
@@ -45,8 +48,12 @@ def expand(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None, sidx
         w = lw[lptr[q]:lptr[q + 1]]
         for p in range(nper):
             r = q * nper + p
-            cols = (k[:, None] * nz + kj0[p] + t[None, :]).reshape(-1)
-            v = (w[:, None] * kern[p][None, :]).reshape(-1)     # one fp64 rounding per value
+            if nodal:
+                cols = (k[:, None] * nz + kj0[k, p][:, None] + t[None, :]).reshape(-1)
+                v = (w[:, None] * kern[k, p, :]).reshape(-1)
+            else:
+                cols = (k[:, None] * nz + kj0[p] + t[None, :]).reshape(-1)
+                v = (w[:, None] * kern[p][None, :]).reshape(-1)     # one fp64 rounding per value
             colind[rowptr[r]:rowptr[r + 1]] = cols
             vals[rowptr[r]:rowptr[r + 1]] = v
     if ms:
@@ -77,14 +84,19 @@ def expand_exact(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr=None
     exact products of both words and round once: the definition  y_i = RN( sum_j (W g)_ij x_j )  written out."""
     rowptr, colind, vals = expand(npairs, nper, nnodes, nz, lptr, lnode, lw, kj0, kern, sptr, sidx, svals)
     lw = np.asarray(lw, dtype=np.float64)
-    kern = np.asarray(kern, dtype=np.float64).reshape(nper, -1)
+    kern = np.asarray(kern, dtype=np.float64)
+    nodal = kern.ndim == 3
+    if not nodal:
+        kern = kern.reshape(nper, -1)
     lptr = np.asarray(lptr, dtype=np.int64)
+    lnode = np.asarray(lnode, dtype=np.int64)
     lo = np.zeros_like(vals)
     for q in range(npairs):
         w = lw[lptr[q]:lptr[q + 1]]
+        k = lnode[lptr[q]:lptr[q + 1]]
         for p in range(nper):
             r = q * nper + p
-            pr, er = two_prod(w[:, None], kern[p][None, :])
+            pr, er = two_prod(w[:, None], kern[k, p, :] if nodal else kern[p][None, :])
             assert np.array_equal(pr.reshape(-1), vals[rowptr[r]:rowptr[r + 1]])
             lo[rowptr[r]:rowptr[r + 1]] = er.reshape(-1)
     return rowptr, colind, vals, lo

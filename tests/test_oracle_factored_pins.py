@@ -19,7 +19,10 @@ def dense_by_definition(f):
             k, w = int(f["lnode"][e]), float(f["lw"][e])
             for p in range(nper):
                 for t in range(klen):
-                    A[q * nper + p, k * nz + int(f["kj0"][p]) + t] = w * float(f["kern"][p][t])
+                    if f["kern"].ndim == 3:   # a kernel table per node
+                        A[q * nper + p, k * nz + int(f["kj0"][k][p]) + t] = w * float(f["kern"][k][p][t])
+                    else:
+                        A[q * nper + p, k * nz + int(f["kj0"][p]) + t] = w * float(f["kern"][p][t])
     for r in range(ms):
         for e in range(f["sptr"][r], f["sptr"][r + 1]):
             A[f["npairs"] * nper + r, f["sidx"][e]] = f["svals"][e]
@@ -163,3 +166,33 @@ def test_exact_entries_lsqr_is_lsqr_on_a_nearby_matrix():
     assert np.array_equal(o0.x, o1.x)
     assert o2.itn == o1.itn == 30 and not np.array_equal(o2.x, o1.x)
     assert np.linalg.norm(o2.x - o1.x) <= 1e-11 * np.linalg.norm(o1.x)
+
+
+@pytest.mark.parametrize("shape", [(7, 3, 9, 6, 4, None), (6, 10, 8, 20, 12, 5)])
+def test_expand_nodal_kernels_is_the_definition(shape):
+    """kernel table per lateral node (the paper's Theta_k): expand and expand_exact against the dense definition"""
+    from fractions import Fraction
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=70 + npairs, ms=ms, nodal=True)
+    rp, ci, va = expand(f)
+    A = dense_by_definition(f)
+    B = np.zeros_like(A)
+    for r in range(A.shape[0]):
+        cols = ci[rp[r]:rp[r + 1]]
+        assert np.all(np.diff(cols) > 0)
+        B[r, cols] = va[rp[r]:rp[r + 1]]
+    assert np.array_equal(A, B)
+    rp2, ci2, va2, lo = factored.expand_exact(f["npairs"], f["nper"], f["nnodes"], f["nz"], f["lptr"], f["lnode"], f["lw"], f["kj0"], f["kern"],
+                                              f["sptr"], f["sidx"], f["svals"])
+    assert np.array_equal(rp2, rp) and np.array_equal(ci2, ci) and np.array_equal(va2, va)
+    e = 0
+    for q in range(npairs):     # the two words add up to the exact product, entry by entry
+        for le in range(f["lptr"][q], f["lptr"][q + 1]):
+            pass
+    for r in range(npairs * nper):
+        q, p = divmod(r, nper)
+        for i, le in enumerate(range(f["lptr"][q], f["lptr"][q + 1])):
+            k = int(f["lnode"][le])
+            for t in range(klen):
+                e = rp[r] + i * klen + t
+                assert Fraction(float(va[e])) + Fraction(float(lo[e])) == Fraction(float(f["lw"][le])) * Fraction(float(f["kern"][k][p][t]))

@@ -251,7 +251,7 @@ def random_csr(m: int, n: int, row_lengths, seed: int, dtype=np.float64):
     return rp, ci, va
 
 
-def random_factored(npairs, nper, nnodes, nz, klen, seed, ms=None, empty_pairs=0.1, empty_nodes=0.1, max_entries=40):
+def random_factored(npairs, nper, nnodes, nz, klen, seed, ms=None, empty_pairs=0.1, empty_nodes=0.1, max_entries=40, nodal=False):
     """Unstructured factored system (unit tests: odd shapes, empty pairs and nodes, windows at the rim): the dict
     :meth:`System.factored` returns, with random footprints, windows and a random short-row extra block (ms rows;
     None: nnodes*nz rows of 0..7 entries; 0: no extra block)."""
@@ -270,6 +270,9 @@ def random_factored(npairs, nper, nnodes, nz, klen, seed, ms=None, empty_pairs=0
     lw[lw == 0] = 1.0
     kj0 = rng.integers(0, nz - klen + 1, size=nper).astype(np.int32)
     kern = rng.standard_normal((nper, klen))
+    if nodal:   # a kernel table per lateral node (the paper's Theta_k): kern[k, p, t], kj0[k, p]
+        kj0 = rng.integers(0, nz - klen + 1, size=(nnodes, nper)).astype(np.int32)
+        kern = rng.standard_normal((nnodes, nper, klen))
     n = nnodes * nz
     if ms is None:
         ms = n
