@@ -131,6 +131,19 @@ tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, int64_t nnode
  * value; the handle is unchanged), CUDA. */
 tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream);
 
+/* Depth kernels that depend on the lateral node (the paper's Theta_k, Eq. 5; BASELINE.json's configs use
+ * one table for all nodes): d_kj0 int32[nnodes * nper] (window start of node k, period p at k * nper + p),
+ * d_kern fp64[nnodes * nper * klen]; same klen as at create; DEVICE arrays, copied into the handle.  From then on
+ *      A_data[q * nper + p, k * nz + j] = W[q, k] * g_{k,p}[j - j0_{k,p}]
+ * and the handle applies it through the depth-contraction kernels in BOTH accumulation modes, whatever "two_stage" says
+ * (a table per node costs the contraction nothing, a per-entry product a table look-up per ray entry): "accumulate" = 1
+ * is then the order-independent iterate on the exact entries (reading F-fac3; bit for bit the dd oracle on two-word
+ * entries), "accumulate" = 0 plain fp64 sums.  May be called again to refresh the tables (the outer loop);
+ * tomo_lsqr_update_kernels is INVALID_ARG afterwards.
+ * Errors: INVALID_ARG (not a factored handle, NULL), NOT_DEVICE_PTR, BAD_CSR (window outside [0, nz), non-finite value;
+ * the handle is unchanged), OOM, CUDA. */
+tomo_status_t tomo_lsqr_set_nodal_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream);
+
 /* NEXT-4: value-only refresh.  The outer Gauss-Newton loop of the inversion
  * re-evaluates G on the same rays and solves again: the sparsity pattern, hence the CSC permutation, the split
  * points and the compressed index, stay; only the values change.  d_vals: device array [nnz] of the handle's value

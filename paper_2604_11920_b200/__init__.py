@@ -23,7 +23,7 @@ TOMO_VAL_F64, TOMO_VAL_F32 = 0, 1
 
 # every symbol include/tomo_lsqr.h declares
 SYMBOLS = (
-    "tomo_lsqr_create", "tomo_lsqr_create_factored", "tomo_lsqr_assemble_csr", "tomo_lsqr_update_kernels", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
+    "tomo_lsqr_create", "tomo_lsqr_create_factored", "tomo_lsqr_assemble_csr", "tomo_lsqr_update_kernels", "tomo_lsqr_set_nodal_kernels", "tomo_lsqr_solve", "tomo_lsmr_solve", "tomo_lsqr_solve_host", "tomo_lsmr_solve_host",
     "tomo_lsqr_solve_multi", "tomo_lsmr_solve_multi", "tomo_lsqr_spmv", "tomo_lsqr_update_values", "tomo_lsqr_solve_sharded",
     "tomo_lsqr_get_csc", "tomo_lsqr_set_option", "tomo_lsqr_get_info", "tomo_lsqr_spmv_noalloc", "tomo_lsqr_destroy", "tomo_status_string",
 )
@@ -62,6 +62,7 @@ def load() -> ctypes.CDLL:
     lib.tomo_lsqr_create_factored.argtypes = [ctypes.POINTER(vp), i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, vp]
     lib.tomo_lsqr_assemble_csr.argtypes = [i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, vp]
     lib.tomo_lsqr_update_kernels.argtypes = [vp, vp, vp, vp]
+    lib.tomo_lsqr_set_nodal_kernels.argtypes = [vp, vp, vp, vp]
     lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
     lib.tomo_lsmr_solve.argtypes = lib.tomo_lsqr_solve.argtypes
     lib.tomo_lsqr_solve_host.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp]
@@ -142,6 +143,12 @@ def tomo_lsqr_update_kernels(h, d_kj0, d_kern, stream=None) -> None:
     st = load().tomo_lsqr_update_kernels(h, _ptr(d_kj0), _ptr(d_kern), _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_update_kernels")
+
+
+def tomo_lsqr_set_nodal_kernels(h, d_kj0, d_kern, stream=None) -> None:
+    st = load().tomo_lsqr_set_nodal_kernels(h, _ptr(d_kj0), _ptr(d_kern), _stream(stream))
+    if st != TOMO_OK:
+        raise TomoError(st, "tomo_lsqr_set_nodal_kernels")
 
 
 def tomo_lsqr_destroy(h) -> None:

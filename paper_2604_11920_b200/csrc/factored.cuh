@@ -39,6 +39,7 @@ struct FacSeg {        // one piece of a node's lateral-CSC entry list, owned by
 
 struct FacDesc {       // uniform kernel argument
   int32_t nper, nz, klen, G;
+  int32_t nodal, pad_;     // 1: kj0 / kern hold a table per lateral node ([nnodes * nper], [nnodes * nper * klen]); two-stage kernels only
   int64_t npairs, nnodes, mdata, ms;
   const int64_t* lptr; const int32_t* lnode; const double* lw;       // W as CSR (pairs x nodes)
   const int64_t* cptr; const int32_t* cpair; const double* cw;       // W as CSC (pairs ascending inside a node)
@@ -397,12 +398,13 @@ k_fac_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ y
 }
 
 // validation of the depth-kernel table: windows inside [0, nz), finite values
-__global__ void k_fac_validate_kern(int nper, int nz, int klen, const int32_t* __restrict__ kj0, const double* __restrict__ kern,
-                                    int* flags) {
+__global__ void k_fac_validate_kern(int64_t nper, int nz, int klen, const int32_t* __restrict__ kj0, const double* __restrict__ kern,
+                                    int* flags) {   // nper: number of windows (periods, or nodes * periods of a nodal table)
   int bad = 0;
-  for (int i = threadIdx.x; i < nper; i += blockDim.x)
+  const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = i0; i < nper; i += stride)
     if (kj0[i] < 0 || kj0[i] + klen > nz) bad = 1;
-  for (int i = threadIdx.x; i < nper * klen; i += blockDim.x)
+  for (int64_t i = i0; i < nper * klen; i += stride)
     if (!(fabs(kern[i]) <= 1.79769313486231570815e308)) bad = 1;
   if (bad) atomicOr(flags, 1);
 }
@@ -484,8 +486,9 @@ __global__ void __launch_bounds__(256) k_fac2_stage(const FacDesc d, const doubl
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int64_t k = i / d.nper;
     const int p = (int)(i - k * d.nper);
-    const double* xp = x + k * d.nz + d.kj0[p];
-    const double* kp = d.kern + (size_t)p * d.klen;
+    const int64_t tab = d.nodal ? i : (int64_t)p;   // the node's own table, or the one all nodes share
+    const double* xp = x + k * d.nz + d.kj0[tab];
+    const double* kp = d.kern + (size_t)tab * d.klen;
     Acc<MODE> s;
     s.zero();
     for (int t = 0; t < d.klen; ++t) s.mac(kp[t], xp[t]);
@@ -692,9 +695,10 @@ k_fac2_cols(const FacDesc d, const double* __restrict__ x, double* __restrict__ 
         Acc<MODE> S;
         S.zero();
         for (int pp = 0; pp < nper; ++pp) {     // the depth contraction: periods ascending
-          const int t = j - s_kj0[pp];
+          const int64_t tab = d.nodal ? (int64_t)node * nper + pp : (int64_t)pp;
+          const int t = j - (d.nodal ? d.kj0[tab] : s_kj0[pp]);
           if (t >= 0 && t < klen) {
-            const double gk = d.kern[(size_t)pp * klen + t];
+            const double gk = d.kern[(size_t)tab * klen + t];
             const double2 Tp = my[pp];
             S.mac(gk, Tp.x);
             if (MODE == 1) S.mac(gk, Tp.y);   // g * (hi + lo): both words as exact products

@@ -78,6 +78,7 @@ struct FacState {
   int nsegs = 0, nslots = 0;
   int64_t* cptr = nullptr; int32_t* cpair = nullptr; double* cw = nullptr;
   int32_t* kj0 = nullptr; double* kern = nullptr;
+  int32_t* kj0n = nullptr; double* kernn = nullptr;   // nodal tables (tomo_lsqr_set_nodal_kernels)
   int64_t* scptr = nullptr; int32_t* srow = nullptr; double* scval = nullptr;
   int32_t* pw = nullptr; int32_t* pq = nullptr; int32_t* pw2 = nullptr; int32_t* pq2 = nullptr; int32_t* wseg[4] = {nullptr, nullptr, nullptr, nullptr}; FacSeg* seg[4] = {nullptr, nullptr, nullptr, nullptr};
   double2* seg_part = nullptr; unsigned int* node_cnt = nullptr; double2* node_nsq = nullptr; long long* busy = nullptr;
@@ -276,6 +277,7 @@ cudaError_t launch_fac2(const tomo_lsqr_s* h, bool cols, const double* x, double
 }
 template <int OP>
 void launch_fac(const tomo_lsqr_s* h, bool transpose, const double* x, double* y, cudaStream_t st) {
+  if (h->fac->d.nodal) { if (h->accumulate) launch_fac2<1, OP>(h, transpose, x, y, st); else launch_fac2<0, OP>(h, transpose, x, y, st); return; }
   if (h->accumulate) { if (h->two_stage == 2) launch_fac2<1, OP>(h, transpose, x, y, st); else launch_fac_mode<1, OP>(h, transpose, x, y, st); }
   else if (h->two_stage) launch_fac2<0, OP>(h, transpose, x, y, st);
   else launch_fac_mode<0, OP>(h, transpose, x, y, st);
@@ -500,7 +502,7 @@ void free_handle(tomo_lsqr_s* h) {
   cudaFree(h->mpartials); if (h->h_msc) cudaFreeHost(h->h_msc); if (h->h_mpoll) cudaFreeHost(h->h_mpoll); if (h->mgexec) cudaGraphExecDestroy(h->mgexec);
   for (Dir& D : h->dir) { cudaFree(D.ptr_own); cudaFree(D.rid); cudaFree(D.erows); cudaFree(D.wE); cudaFree(D.wR); cudaFree(D.cidx); cudaFree(D.coff); }
   if (FacState* f = h->fac) {
-    cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern);
+    cudaFree(f->cptr); cudaFree(f->cpair); cudaFree(f->cw); cudaFree(f->kj0); cudaFree(f->kern); cudaFree(f->kj0n); cudaFree(f->kernn);
     cudaFree(f->scptr); cudaFree(f->srow); cudaFree(f->scval); cudaFree(f->pw); cudaFree(f->pq); cudaFree(f->pw2); cudaFree(f->pq2); cudaFree(f->S2); for (int i = 0; i < 4; ++i) { cudaFree(f->wseg[i]); cudaFree(f->seg[i]); }
     cudaFree(f->seg_part); cudaFree(f->node_cnt); cudaFree(f->node_nsq); cudaFree(f->busy);
     delete f;
@@ -676,7 +678,7 @@ extern "C" tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npa
     cudaMemsetAsync(d_flags, 0, sizeof(int), st);
     k_validate<double><<<sms * 8, kThreads, 0, st>>>(npairs, nnodes, E, d_lptr, d_lnode, d_lw, d_flags);
     if (ms > 0) k_validate<double><<<sms * 8, kThreads, 0, st>>>(ms, n, snnz, d_sptr, d_sidx, d_svals, d_flags);
-    k_fac_validate_kern<<<1, 256, 0, st>>>(nper, nz, klen, d_kj0, d_kern, d_flags);
+    k_fac_validate_kern<<<1, 256, 0, st>>>((int64_t)nper, nz, klen, d_kj0, d_kern, d_flags);
     int flags = 0;
     if ((e = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
         (e = cudaStreamSynchronize(st)) != cudaSuccess) { rc = cuda_fail(e, "validation of the factored operator"); break; }
@@ -996,7 +998,7 @@ tomo_status_t solve_device(tomo_lsqr_s* h, const double* d_b, double damp, doubl
       }
       CK(cudaGetLastError());
     }
-    h->kernels_enqueued += (h->fac && (h->accumulate ? h->two_stage == 2 : h->two_stage != 0) ? 4.0 : 3.0) * k;   // the two-stage A x is two launches
+    h->kernels_enqueued += (h->fac && (h->fac->d.nodal || (h->accumulate ? h->two_stage == 2 : h->two_stage != 0)) ? 4.0 : 3.0) * k;   // the two-stage A x is two launches
     // host poll: {itn, istop, stop}.  The next replay is enqueued before this one is inspected, so the
     // device never idles on the host; kernels after a stop return at once and leave x frozen.
     CK(cudaMemcpyAsync(&h->h_poll[slot], &h->sc->itn, sizeof(PollWord), cudaMemcpyDeviceToHost, st));
@@ -1397,8 +1399,44 @@ tomo_status_t update_values_t(tomo_lsqr_s* h, const VT* d_vals, cudaStream_t st)
 }  // namespace
 
 // NEXT-4 for the factored form: new depth kernels on the same rays
-extern "C" tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream) {
+// a kernel table per lateral node (the paper's Theta_k): the handle applies it through the two-stage kernels
+extern "C" tomo_status_t tomo_lsqr_set_nodal_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream) {
   if (!h || !h->fac || !d_kj0 || !d_kern) return TOMO_ERR_INVALID_ARG;
+  { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
+  if (!is_device_ptr(d_kj0) || !is_device_ptr(d_kern)) return TOMO_ERR_NOT_DEVICE_PTR;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  FacState* f = h->fac;
+  const int64_t ntab = f->d.nnodes * f->d.nper;
+  const int klen = f->d.klen, nz = f->d.nz;
+  int* d_flags = nullptr;
+  CK(cudaMalloc(&d_flags, sizeof(int)));
+  cudaMemsetAsync(d_flags, 0, sizeof(int), st);
+  k_fac_validate_kern<<<h->sms * 4, 256, 0, st>>>(ntab, nz, klen, d_kj0, d_kern, d_flags);
+  int flags = 0;
+  cudaError_t e = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_flags);
+  if (e != cudaSuccess) return cuda_fail(e, "validation of the nodal kernel table");
+  if (flags) return TOMO_ERR_BAD_CSR;   // nothing has been touched
+  if (!f->kj0n) {
+    int32_t* a = nullptr; double* b2 = nullptr;
+    if ((e = cudaMalloc(&a, sizeof(int32_t) * ntab)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(nodal windows)");
+    if ((e = cudaMalloc(&b2, sizeof(double) * ntab * klen)) != cudaSuccess) { cudaFree(a); return cuda_fail(e, "cudaMalloc(nodal kernels)"); }
+    f->kj0n = a; f->kernn = b2;
+  }
+  CK(cudaMemcpyAsync(f->kj0n, d_kj0, sizeof(int32_t) * ntab, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(f->kernn, d_kern, sizeof(double) * ntab * klen, cudaMemcpyDeviceToDevice, st));
+  CK(cudaStreamSynchronize(st));
+  if (!f->d.nodal) {   // the kernel argument changes: captured graphs hold the old one
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    f->d.nodal = 1; f->d.kj0 = f->kj0n; f->d.kern = f->kernn;
+    for (int mode = 0; mode < 4; ++mode) { f->dm[mode].nodal = 1; f->dm[mode].kj0 = f->kj0n; f->dm[mode].kern = f->kernn; }
+  }
+  return TOMO_OK;
+}
+
+extern "C" tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* d_kj0, const double* d_kern, void* cuda_stream) {
+  if (!h || !h->fac || h->fac->d.nodal || !d_kj0 || !d_kern) return TOMO_ERR_INVALID_ARG;
   { tomo_status_t rc = check_device(h); if (rc != TOMO_OK) return rc; }
   if (!is_device_ptr(d_kj0) || !is_device_ptr(d_kern)) return TOMO_ERR_NOT_DEVICE_PTR;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1407,7 +1445,7 @@ extern "C" tomo_status_t tomo_lsqr_update_kernels(tomo_lsqr_t h, const int32_t* 
   int* d_flags = nullptr;
   CK(cudaMalloc(&d_flags, sizeof(int)));
   cudaMemsetAsync(d_flags, 0, sizeof(int), st);
-  k_fac_validate_kern<<<1, 256, 0, st>>>(nper, nz, klen, d_kj0, d_kern, d_flags);
+  k_fac_validate_kern<<<1, 256, 0, st>>>((int64_t)nper, nz, klen, d_kj0, d_kern, d_flags);
   int flags = 0;
   cudaError_t e = cudaMemcpyAsync(&flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -1599,6 +1637,7 @@ extern "C" tomo_status_t tomo_lsqr_get_info(tomo_lsqr_t h, const char* key, doub
   const double vb = h->vt == TOMO_VAL_F64 ? 8.0 : 4.0;
   if (k == "create_ms") *out = h->create_ms;
   else if (k == "factored") *out = h->fac ? 1.0 : 0.0;
+  else if (k == "nodal_kernels") *out = (h->fac && h->fac->d.nodal) ? 1.0 : 0.0;
   else if (k == "lateral_entries") *out = h->fac ? (double)h->fac->E : 0.0;
   else if (k == "cut_nodes_pieces") *out = h->fac ? (double)h->fac->nslots : 0.0;
   else if (k == "operator_bytes")   // what a product has to read of the operator itself

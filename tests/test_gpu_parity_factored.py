@@ -449,3 +449,46 @@ def test_update_kernels_equals_create_from_scratch(tl):
     with pytest.raises(T.TomoError):
         T.tomo_lsqr_update_kernels(C.h, dev(g["kj0"]), dev(g["kern"]))   # not a factored handle
     C.close(); S.close(); R.close()
+
+
+@pytest.mark.parametrize("shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[4], SHAPES[7]])
+def test_nodal_kernel_tables(tl, shape):
+    """Depth kernels per lateral node (the paper's Theta_k) through tomo_lsqr_set_nodal_kernels: dd mode bitwise the
+    dd oracle on the exact two-word entries, fast mode to the SpMV bar against the plain oracle on the multiplied-out
+    matrix; refresh of the tables; a bad table leaves the handle unchanged."""
+    import paper_2604_11920_b200 as T
+    npairs, nper, nnodes, nz, klen, ms = shape
+    f = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=4000 + npairs, ms=ms, max_entries=60, nodal=True)
+    rp, ci, va, lo = expand_exact(f)
+    m, n = len(rp) - 1, nnodes * nz
+    shared = dict(f); shared["kj0"] = f["kj0"][0].copy(); shared["kern"] = f["kern"][0].copy()
+    S = make(tl, shared)
+    T.tomo_lsqr_set_nodal_kernels(S.h, dev(f["kj0"].astype(np.int32)), dev(f["kern"]))
+    assert S.info("nodal_kernels") == 1.0
+    rng = np.random.default_rng(npairs)
+    x, u, b = rng.standard_normal(n), rng.standard_normal(m), rng.standard_normal(m)
+    S.set(accumulate=1)
+    assert np.array_equal(S.spmv(dev(x)).cpu().numpy(), oracle.spmv(m, n, rp, ci, va, x, oracle.DD, vals_lo=lo))
+    assert np.array_equal(S.spmv(dev(u), transpose=True).cpu().numpy(), oracle.spmv_t(m, n, rp, ci, va, u, oracle.DD, vals_lo=lo))
+    xg, res = S.solve(dev(b), damp=0.1, max_iters=20)
+    o = oracle.lsqr(m, n, rp, ci, va, b, damp=0.1, max_iters=20, mode=oracle.DD, vals_lo=lo)
+    assert (res.itn, res.istop) == (o.itn, o.istop) and np.array_equal(xg.cpu().numpy(), o.x)
+    S.set(accumulate=0)
+    assert rel(S.spmv(dev(x)).cpu().numpy(), oracle.spmv(m, n, rp, ci, va, x, oracle.PLAIN)) <= 1e-11
+    assert rel(S.spmv(dev(u), transpose=True).cpu().numpy(), oracle.spmv_t(m, n, rp, ci, va, u, oracle.PLAIN)) <= 1e-11
+    # refresh with other tables: equals a handle that got them first
+    g = tomogen.random_factored(npairs, nper, nnodes, nz, klen, seed=4000 + npairs, ms=ms, max_entries=60, nodal=True)
+    g["kern"] = np.random.default_rng(5).standard_normal(f["kern"].shape)
+    bad = g["kern"].copy(); bad[-1, -1, -1] = np.nan
+    with pytest.raises(T.TomoError) as ei:
+        T.tomo_lsqr_set_nodal_kernels(S.h, dev(g["kj0"].astype(np.int32)), dev(bad))
+    assert ei.value.status == T.TOMO_ERR_BAD_CSR
+    S.set(accumulate=1)
+    assert np.array_equal(S.solve(dev(b), damp=0.1, max_iters=20)[0].cpu().numpy(), o.x)
+    T.tomo_lsqr_set_nodal_kernels(S.h, dev(g["kj0"].astype(np.int32)), dev(g["kern"]))
+    rp2, ci2, va2, lo2 = expand_exact(g)
+    o2 = oracle.lsqr(m, n, rp2, ci2, va2, b, damp=0.1, max_iters=20, mode=oracle.DD, vals_lo=lo2)
+    assert np.array_equal(S.solve(dev(b), damp=0.1, max_iters=20)[0].cpu().numpy(), o2.x)
+    with pytest.raises(T.TomoError):
+        T.tomo_lsqr_update_kernels(S.h, dev(shared["kj0"].astype(np.int32)), dev(shared["kern"]))
+    S.close()
