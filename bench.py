@@ -148,7 +148,9 @@ def workload_config(s, args, iterations_per_step: int, world: int = 1) -> dict:
             "accumulate": ("dd (double-double sums, rounded once)" if args.accumulate else "fast (fp64 FMA sums)") +
                           (("; factored operator with exact entries W*g, depth contraction first (two_stage=2)" if args.accumulate else
                             "; depth contraction first (two_stage)") if getattr(args, "factored", 0) and
-                           (getattr(args, "two_stage", 1) == 2 or (not args.accumulate and getattr(args, "two_stage", 1) >= 1)) else ""),
+                           (getattr(args, "nodal", 0) or getattr(args, "two_stage", 1) == 2 or
+                            (not args.accumulate and getattr(args, "two_stage", 1) >= 1)) else "") +
+                          ("; kernel table per lateral node" if getattr(args, "factored", 0) and getattr(args, "nodal", 0) else ""),
             "check_every": args.check_every, "solver": args.solver, "right_hand_sides": nrhs,
             "values": "fp64" if vbytes == 8 else "fp32 storage, fp64 arithmetic",
             "index": ("none: factored operator (lateral footprint x depth kernel, tomo_lsqr_create_factored)" if getattr(args, "factored", 0)
@@ -245,6 +247,12 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
     S.set(accumulate=args.accumulate, check_every=args.check_every, graph=1, profile=0, compress=0 if factored else args.compress)
     if factored:
         S.set(two_stage=getattr(args, "two_stage", 1))
+        if getattr(args, "nodal", 0):
+            # a kernel table per lateral node (the paper's Theta_k): here the shared table repeated for every node, so the
+            # operator is the same and only the kernel path changes (the depth-contraction kernels in both modes)
+            kj0n = ft["kj0"].repeat(f["nnodes"], 1).contiguous()
+            kernn = ft["kern"].unsqueeze(0).repeat(f["nnodes"], 1, 1).contiguous()
+            tl.tomo_lsqr_set_nodal_kernels(S.h, kj0n, kernn)
     if args.row_cost is not None:
         S.set(row_cost=args.row_cost)
     if args.pdl is not None:
@@ -299,6 +307,7 @@ def measure(tl, torch, s, args, barrier, dist, world, steps, warmup, e2e=True, b
            "create_ms": S.info("create_ms"), "transpose_ms": S.info("transpose_ms")}
     if factored:
         out["two_stage"] = getattr(args, "two_stage", 1)
+        out["nodal"] = getattr(args, "nodal", 0)
         out["factored"] = {"lateral_entries": S.info("lateral_entries"), "operator_bytes": S.info("operator_bytes"),
                            "cut_nodes_pieces": S.info("cut_nodes_pieces")}
         if torch.cuda.mem_get_info()[0] > 14 * nnz + (2 << 30):
@@ -442,7 +451,7 @@ def roofline_of(r: dict, peak: float, peak_src: str, compress: int) -> dict:
         # fl(W g) 1 + TwoProd 2 + TwoSum 6 + 2 error adds; fast 2 = the value + the FMA.  Peak as for the dd block solve.
         per = 11.0 if r.get("accumulate", 1) == 1 else 2.0
         two = r.get("two_stage", 1)
-        contracted = (two == 2) if r.get("accumulate", 1) == 1 else (two >= 1)
+        contracted = r.get("nodal", 0) or ((two == 2) if r.get("accumulate", 1) == 1 else (two >= 1))
         sm_max = (r.get("clocks") or {}).get("sm_max_mhz") or 1965.0
         peak_t = 148 * 64 * sm_max * 1e6 / 1e12
         ach_t = per * nnz * 2 / ((r["k1_us"] + r["k2_us"]) * 1e-6) / 1e12
@@ -649,6 +658,7 @@ def main():
     ap.add_argument("--two-stage", dest="two_stage", type=int, default=1, choices=[0, 1, 2],
                     help="factored operator: 0 per-entry products in both modes, 1 (default) depth contraction first in fast mode, "
                          "2 also in dd mode (exact entries W*g, DESIGN.md F-fac3)")
+    ap.add_argument("--nodal", type=int, default=0, choices=[0, 1], help="factored operator: install a kernel table per lateral node (tomo_lsqr_set_nodal_kernels)")
     ap.add_argument("--row-cost", dest="row_cost", type=int, default=None, help="tuning: per-row weight of the element split")
     ap.add_argument("--pdl", type=int, default=None, choices=[0, 1], help="tuning: programmatic dependent launch between the kernels of an iteration")
     ap.add_argument("--shards", type=int, default=0, help="NEXT-3: P row blocks solved by tomo_lsqr_solve_sharded (one GPU: all blocks local; torchrun: one block per rank)")
