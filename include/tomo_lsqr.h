@@ -7,8 +7,10 @@
  *
  * by LSQR (Golub-Kahan bidiagonalisation, Paige & Saunders 1982) with x_0 = 0.  A stacks the
  * traveltime-sensitivity rows (Eq. 1, Eq. 5, unknowns depth-fastest Eq. 7) on top
- * of smoothing rows; the library itself accepts any canonical CSR matrix.  The step-by-step algorithm,
- * the stopping rules and every reading taken where the paper is silent are in DESIGN.md.
+ * of smoothing rows; the library itself accepts any canonical CSR matrix, or the sensitivity block in the factored
+ * form of Eq. 5 (ray footprint x depth kernel: tomo_lsqr_create_factored, tomo_lsqr_set_nodal_kernels,
+ * tomo_lsqr_update_kernels, tomo_lsqr_assemble_csr).  The step-by-step algorithm, the stopping rules and every reading
+ * taken where the paper is silent are in DESIGN.md.
  *
  * Everything runs in hand-written CUDA kernels for sm_100a (no cuSPARSE/cuBLAS, no CPU fallback):
  * a device-side stable CSR->CSC transpose at create, fused SpMV+axpy+norm kernels for A v and A^T u,
