@@ -115,14 +115,16 @@ tomo_status_t tomo_lsqr_create_factored(tomo_lsqr_t* out, int64_t npairs, int32_
  * fully overwritten; nnz must equal d_lptr[npairs] * nper * klen + snnz (INVALID_ARG otherwise, nothing written).
  * Row q * nper + p holds, for the pair's lateral entries in order, value fl(W[q, k] * g_p[t]) at column k * nz + j0_p + t
  * (t = 0 .. klen - 1); the extra block follows unchanged.  The inputs are NOT validated here (tomo_lsqr_create on the
- * result validates the matrix).  One HBM-bound pass: 12 bytes written per nonzero.  The outer Gauss-Newton loop
+ * result validates the matrix).  nodal = 1: d_kj0 / d_kern hold a table per lateral node (int32[nnodes * nper],
+ * fp64[nnodes * nper * klen], as tomo_lsqr_set_nodal_kernels takes them; the paper's Theta_k); 0: one table for all
+ * nodes.  One HBM-bound pass: 12 bytes written per nonzero.  The outer Gauss-Newton loop
  * re-evaluates the depth kernels every iteration: this call (or tomo_lsqr_create_factored, which needs no assembly at all)
  * replaces the host-side assembly.  Errors: INVALID_ARG, RANGE, NOT_DEVICE_PTR, UNSUPPORTED_ARCH, CUDA. */
 tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, int64_t nnodes, int32_t nz, const int64_t* d_lptr,
                                      const int32_t* d_lnode, const double* d_lw, int32_t klen, const int32_t* d_kj0,
                                      const double* d_kern, int64_t ms, int64_t snnz, const int64_t* d_sptr, const int32_t* d_sidx,
                                      const double* d_svals, int64_t nnz, int64_t* d_rowptr, int32_t* d_colind, double* d_vals,
-                                     void* cuda_stream);
+                                     int32_t nodal, void* cuda_stream);
 
 /* NEXT-4 for a factored handle: new depth kernels on the same rays.  The outer Gauss-Newton loop
  * re-evaluates the depth kernels of the updated model and solves again; W (the rays' lateral footprints), its transpose

@@ -60,7 +60,7 @@ def load() -> ctypes.CDLL:
     vp, i64, i32, f64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int
     lib.tomo_lsqr_create.argtypes = [ctypes.POINTER(vp), i64, i64, i64, vp, vp, vp, ci, vp]
     lib.tomo_lsqr_create_factored.argtypes = [ctypes.POINTER(vp), i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, vp]
-    lib.tomo_lsqr_assemble_csr.argtypes = [i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, vp]
+    lib.tomo_lsqr_assemble_csr.argtypes = [i64, i32, i64, i32, vp, vp, vp, i32, vp, vp, i64, i64, vp, vp, vp, i64, vp, vp, vp, i32, vp]
     lib.tomo_lsqr_update_kernels.argtypes = [vp, vp, vp, vp]
     lib.tomo_lsqr_set_nodal_kernels.argtypes = [vp, vp, vp, vp]
     lib.tomo_lsqr_solve.argtypes = [vp, vp, f64, f64, f64, i32, vp, ctypes.POINTER(tomo_lsqr_result_t), vp, vp, vp]
@@ -130,11 +130,11 @@ def tomo_lsqr_create_factored(npairs, nper, nnodes, nz, d_lptr, d_lnode, d_lw, k
 
 
 def tomo_lsqr_assemble_csr(npairs, nper, nnodes, nz, d_lptr, d_lnode, d_lw, klen, d_kj0, d_kern, ms, snnz, d_sptr, d_sidx, d_svals,
-                           nnz, d_rowptr, d_colind, d_vals, stream=None) -> None:
-    """The factored description multiplied out into CSR device arrays (on-device assembly of G)."""
+                           nnz, d_rowptr, d_colind, d_vals, stream=None, nodal=0) -> None:
+    """The factored description multiplied out into CSR device arrays (on-device assembly of G).  nodal=1: a kernel table per node."""
     st = load().tomo_lsqr_assemble_csr(int(npairs), int(nper), int(nnodes), int(nz), _ptr(d_lptr), _ptr(d_lnode), _ptr(d_lw), int(klen),
                                        _ptr(d_kj0), _ptr(d_kern), int(ms), int(snnz), _ptr(d_sptr), _ptr(d_sidx), _ptr(d_svals),
-                                       int(nnz), _ptr(d_rowptr), _ptr(d_colind), _ptr(d_vals), _stream(stream))
+                                       int(nnz), _ptr(d_rowptr), _ptr(d_colind), _ptr(d_vals), int(nodal), _stream(stream))
     if st != TOMO_OK:
         raise TomoError(st, "tomo_lsqr_assemble_csr")
 

@@ -419,7 +419,7 @@ namespace tomo {
 // nper rows are cnt * klen elements each and contiguous, so the stores are coalesced; W is read through L1.
 // value = fl(W[q, k] * g_p[t]) (one rounding), column = k * nz + j0_p + t.  HBM-bound: 12 bytes written per nonzero.
 // ------------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, int nz, int klen, const int64_t* __restrict__ lptr,
+__global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, int nz, int klen, int nodal, const int64_t* __restrict__ lptr,
                                                       const int32_t* __restrict__ lnode, const double* __restrict__ lw,
                                                       const int32_t* __restrict__ kj0, const double* __restrict__ kern, int64_t ms,
                                                       const int64_t* __restrict__ sptr, const int32_t* __restrict__ sidx,
@@ -442,8 +442,15 @@ __global__ void __launch_bounds__(256) k_fac_assemble(int64_t npairs, int nper, 
       int64_t i = lane / klen;
       int t = lane - (int)i * klen;
       for (int64_t idx = lane; idx < rowlen; idx += 32) {
-        colind[out + idx] = lnode[e0 + i] * nz + j0 + t;
-        vals[out + idx] = lw[e0 + i] * kp[t];
+        const int node = lnode[e0 + i];
+        if (nodal) {   // the node's own table (kj0[k * nper + p], kern[(k * nper + p) * klen + t])
+          const int64_t tab = (int64_t)node * nper + p;
+          colind[out + idx] = node * nz + kj0[tab] + t;
+          vals[out + idx] = lw[e0 + i] * kern[tab * klen + t];
+        } else {
+          colind[out + idx] = node * nz + j0 + t;
+          vals[out + idx] = lw[e0 + i] * kp[t];
+        }
         i += di; t += dt;
         if (t >= klen) { t -= klen; ++i; }
       }

@@ -867,7 +867,8 @@ extern "C" tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, in
                                                 const int32_t* d_lnode, const double* d_lw, int32_t klen, const int32_t* d_kj0,
                                                 const double* d_kern, int64_t ms, int64_t snnz, const int64_t* d_sptr,
                                                 const int32_t* d_sidx, const double* d_svals, int64_t nnz, int64_t* d_rowptr,
-                                                int32_t* d_colind, double* d_vals, void* cuda_stream) {
+                                                int32_t* d_colind, double* d_vals, int32_t nodal, void* cuda_stream) {
+  if (nodal != 0 && nodal != 1) return TOMO_ERR_INVALID_ARG;
   if (npairs < 1 || nnodes < 1 || nz < 1 || nper < 1 || klen < 1 || ms < 0 || snnz < 0 || nnz < 0) return TOMO_ERR_INVALID_ARG;
   if (nper > 32 || klen > 32 || klen > nz) return TOMO_ERR_RANGE;
   if ((double)npairs * nper + (double)ms >= (double)INT32_MAX || (double)nnodes * nz >= (double)INT32_MAX) return TOMO_ERR_RANGE;
@@ -892,7 +893,7 @@ extern "C" tomo_status_t tomo_lsqr_assemble_csr(int64_t npairs, int32_t nper, in
   if (E < 0 || sn != snnz || E * (int64_t)nper * klen + snnz != nnz) return TOMO_ERR_INVALID_ARG;
   if (E > 0 && (!d_lnode || !d_lw)) return TOMO_ERR_INVALID_ARG;
   if (E > 0 && (!is_device_ptr(d_lnode) || !is_device_ptr(d_lw))) return TOMO_ERR_NOT_DEVICE_PTR;
-  k_fac_assemble<<<sms * 8, 256, 0, st>>>(npairs, nper, nz, klen, d_lptr, d_lnode, d_lw, d_kj0, d_kern, ms, d_sptr, d_sidx, d_svals,
+  k_fac_assemble<<<sms * 8, 256, 0, st>>>(npairs, nper, nz, klen, (int)nodal, d_lptr, d_lnode, d_lw, d_kj0, d_kern, ms, d_sptr, d_sidx, d_svals,
                                          d_rowptr, d_colind, d_vals);
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(st));
