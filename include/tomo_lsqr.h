@@ -93,8 +93,8 @@ tomo_status_t tomo_lsqr_create(tomo_lsqr_t* out, int64_t m, int64_t n, int64_t n
  * m = npairs * nper + ms < 2^31, n = nnodes * nz < 2^31.  BORROWED until destroy: d_lptr, d_lnode, d_lw, d_sptr, d_sidx,
  * d_svals; d_kj0 and d_kern are copied.  The handle owns W by node (CSC), A_extra by column, the static work split.
  * A lateral entry (12 bytes) stands for nper * klen nonzeros of the CSR form, so the products are bound by fp64
- * arithmetic instead of HBM (get_info "operator_bytes").  Every product uses the ROUNDED value fl(W g), the number the
- * CSR form stores: with "accumulate" = 1 all results (tomo_lsqr_spmv, the solves) are bit for bit those of a
+ * arithmetic instead of HBM (get_info "operator_bytes").  With default options every dd product uses the ROUNDED value
+ * fl(W g), the number the CSR form stores: with "accumulate" = 1 all results (tomo_lsqr_spmv, the solves) are bit for bit those of a
  * tomo_lsqr_create handle on the expanded matrix; with "accumulate" = 0 they agree to rounding (other summation order and,
  * with option "two_stage" = 1, the unrounded entries W g).
  * Supported on such a handle: tomo_lsqr_solve / tomo_lsmr_solve, *_solve_host, *_solve_multi (the sides run one after
